@@ -1,0 +1,141 @@
+/*
+ * rmsynth.h -- C-ABI boundary of librmsynth.so: Faraday rotation-measure synthesis on one
+ * NVIDIA B200 (sm_100a).  Operation (arxiv 1810.06250; P:L<n> = line n of PAPER.md):
+ *
+ *   F(phi_k) = K sum_i w_i (Q_i + iU_i) exp(-2i phi_k (lambda_i^2 - lambda_0^2))    Eq. 11
+ *   FQ = K sum_i w_i (Q_i cos th_ik + U_i sin th_ik)                                Eq. 15/18
+ *   FU = K sum_i w_i (U_i cos th_ik - Q_i sin th_ik)                                Eq. 16/19
+ *   th_ik = 2 phi_k (lambda_i^2 - lambda_0^2),  K = 1/sum w_i (Eq. 13),
+ *   lambda_i^2 = (c/nu_i)^2,  lambda_0^2 = K sum w_i lambda_i^2 (weighted-mean reading)
+ *   R(phi) = K sum_i w_i exp(-2i phi (lambda_i^2 - lambda_0^2))                     Eq. 12
+ *
+ * for every line of sight (pixel) of a Q/U cube.  The weights multiply every term (they are
+ * the W(lambda^2) of Eq. 7).  All entry points return an rmsynth_status; nothing
+ * throws or aborts.  The library never falls back to the CPU: without a usable sm_100
+ * device every compute call fails with RMSYNTH_EUNSUPPORTED / RMSYNTH_ECUDA.
+ *
+ * Ownership: the caller owns every buffer it passes.  A plan owns only what it allocated
+ * and is immutable after creation.  Inputs are never modified.  Q/U must not alias FQ/FU.
+ * Cube pointers need 4-byte alignment only (16-byte alignment enables the TMA fast paths).
+ */
+#ifndef RMSYNTH_H
+#define RMSYNTH_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rmsynth_plan rmsynth_plan; /* opaque */
+
+typedef enum {
+    RMSYNTH_OK = 0,
+    RMSYNTH_EINVAL = 1,       /* bad argument (see each call)                          */
+    RMSYNTH_ENOMEM = 2,       /* host or device allocation failed                      */
+    RMSYNTH_ECUDA = 3,        /* a CUDA call failed; text in rmsynth_last_error()      */
+    RMSYNTH_EUNSUPPORTED = 4  /* device is not compute capability 10.x, or the scheme   */
+                              /* cannot serve this shape/alignment                      */
+} rmsynth_status;
+
+/* layout = one RMSYNTH_IN_* | one RMSYNTH_OUT_*.  p = y*NX + x is the pixel index.
+ *   IN_LOS_MAJOR   Q[p*n_chan + i]   (frequency fastest; cuFFS "rotated" cubes)
+ *   IN_FREQ_MAJOR  Q[i*n_pix + p]    (FITS order, frequency slowest)
+ *   OUT_LOS_MAJOR  F[p*n_phi + k]    (phi fastest: the paper's output order)
+ *   OUT_PHI_MAJOR  F[k*n_pix + p]    (phi as third/slowest axis: after the paper's
+ *                                     "derotation", Table 1 note (c))           */
+enum {
+    RMSYNTH_IN_LOS_MAJOR = 0,
+    RMSYNTH_IN_FREQ_MAJOR = 1,
+    RMSYNTH_OUT_LOS_MAJOR = 0,
+    RMSYNTH_OUT_PHI_MAJOR = 2
+};
+
+/* Arithmetic scheme of the contraction (rows a5/a9 of the scope table).              */
+enum {
+    RMSYNTH_SCHEME_AUTO = 0,        /* = 3xTF32 tensor cores                             */
+    RMSYNTH_SCHEME_TF32X3 = 1,      /* tcgen05 tensor cores, split-precision 3xTF32,     */
+                                    /* FP32 accumulate in TMEM                           */
+    RMSYNTH_SCHEME_FP32_TABLE = 3,  /* CUDA cores, FP32 FMA, reads the plan's cos/sin    */
+    RMSYNTH_SCHEME_FP32_SINCOS = 4  /* CUDA cores, sincos on the fly, one (pixel,phi)    */
+                                    /* per thread -- the paper's kernel shape    */
+};
+
+typedef struct {
+    int struct_size;   /* sizeof(rmsynth_options); lets the struct grow                   */
+    int scheme;        /* RMSYNTH_SCHEME_*                                                */
+    int lambda0_mode;  /* 0 weighted mean (default), 1 plain mean, 2 explicit lambda0_sq  */
+    int device;        /* CUDA device ordinal, -1 = current device                        */
+    double lambda0_sq; /* used when lambda0_mode == 2 (0 reproduces Fig. 1 left)  */
+} rmsynth_options;
+
+/* Build a plan: lambda_i^2, K, lambda_0^2 on the host in FP64 ("computed only once"),
+ * then on the device the FP64 sincos phase matrix K w_i cos/sin th_ik, rounded to the
+ * scheme's operand format, and R(phi) on the plan grid (Eq. 12).
+ *   nu_hz[n_chan]  HOST, channel centre frequencies in Hz, finite and > 0
+ *   w[n_chan]      HOST, weights >= 0, finite, sum > 0; NULL = all ones
+ *   phi[n_phi]     HOST, Faraday depths in rad m^-2, finite, any order or spacing
+ *   opt            NULL = defaults
+ * Host arrays are copied.  Synchronous.  EINVAL on n_chan < 1, n_phi < 1, NULL plan/nu/phi,
+ * bad values, unknown scheme/mode. */
+rmsynth_status rmsynth_plan_create(rmsynth_plan **plan, const double *nu_hz, const double *w,
+                                   int n_chan, const double *phi, int n_phi,
+                                   const rmsynth_options *opt);
+rmsynth_status rmsynth_plan_destroy(rmsynth_plan *plan); /* NULL is a no-op */
+
+/* Scalars of the plan (any out pointer may be NULL). */
+rmsynth_status rmsynth_plan_info(const rmsynth_plan *plan, double *lambda0_sq, double *K,
+                                 int *n_chan, int *n_phi, int *scheme);
+
+/* Copy the plan's FP32-rounded phase matrix to HOST arrays cos_kw[n_chan*n_phi],
+ * sin_kw[n_chan*n_phi], index i*n_phi + k, value K w_i cos/sin th_ik (either may be NULL).
+ * For tests of row a2.  Synchronous. */
+rmsynth_status rmsynth_plan_phase_matrix(const rmsynth_plan *plan, float *cos_kw, float *sin_kw);
+
+/* Eqs. 15-16 for n_pix lines of sight.
+ *   Q, U    DEVICE, n_pix*n_chan floats each, input layout per `layout`
+ *   FQ, FU  DEVICE, n_pix*n_phi floats each, output layout per `layout`
+ *   stream  a cudaStream_t (NULL = default stream).  The call only enqueues work; it never
+ *           synchronises and never allocates after the plan's first use on a shape.
+ * n_pix == 0 is a successful no-op.  EINVAL: n_pix < 0, NULL Q/U/FQ/FU, unknown layout bits.
+ * Non-finite samples propagate to the outputs of their pixel (no masking). */
+rmsynth_status rmsynth_execute(const rmsynth_plan *plan, const float *Q, const float *U,
+                               long long n_pix, int layout, float *FQ, float *FU, void *stream);
+
+/* rmsynth_execute plus the fused peak epilogue (Eq. 14, Eq. 17):
+ * per pixel k* = argmax_k |F_k| (lowest k on ties, |F| compared in FP32), three-point
+ * parabolic refinement of (phi, |F|) on the plan's grid (none at the grid edges or when the
+ * three points are not strictly concave), and
+ *   pa_lambda0 = 0.5 atan2(FU_k*, FQ_k*)                      angle at lambda_0^2
+ *   pa_zero    = pa_lambda0 - peak_phi * lambda_0^2           wrapped to [-pi/2, pi/2)
+ * FQ/FU may both be NULL (maps only).  Each map is DEVICE [n_pix] and may be NULL;
+ * peak_index (int) receives k*. */
+rmsynth_status rmsynth_execute_peaks(const rmsynth_plan *plan, const float *Q, const float *U,
+                                     long long n_pix, int layout, float *FQ, float *FU,
+                                     float *peak_amp, float *peak_phi, float *pa_lambda0,
+                                     float *pa_zero, int *peak_index, void *stream);
+
+/* Same as rmsynth_execute_peaks with every cube/map pointer in HOST memory (pinned memory
+ * gives full PCIe rate): the library streams pixel chunks host->device->host through its own
+ * device buffers, overlapping copies with compute, and returns when the outputs are complete.
+ * Each datum crosses the bus once (the paper's transfer rule).  Synchronous. */
+rmsynth_status rmsynth_execute_host(const rmsynth_plan *plan, const float *Q, const float *U,
+                                    long long n_pix, int layout, float *FQ, float *FU,
+                                    float *peak_amp, float *peak_phi, float *pa_lambda0,
+                                    float *pa_zero, int *peak_index);
+
+/* R(phi) of Eq. 12 in FP64.  phi_eval HOST [n] or NULL for the plan grid (then n must be
+ * n_phi); R_re, R_im HOST [n].  Synchronous. */
+rmsynth_status rmsynth_rmsf(const rmsynth_plan *plan, const double *phi_eval, int n,
+                            double *R_re, double *R_im);
+
+/* Number of kernels this library has launched in this process (for bench.py's
+ * gpu_launches claim); pass reset != 0 to zero the counter after reading. */
+long long rmsynth_launch_count(int reset);
+
+const char *rmsynth_strerror(rmsynth_status s);
+const char *rmsynth_last_error(void); /* thread-local detail of the last failure */
+const char *rmsynth_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RMSYNTH_H */

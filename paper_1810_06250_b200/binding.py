@@ -1,0 +1,137 @@
+"""Thin ctypes binding of librmsynth.so: argument marshalling only, same names as include/rmsynth.h.
+
+Every step of the hot path runs in the library's CUDA kernels; torch is used by callers for
+device memory and streams only.  There is no CPU fallback: if the library is missing this
+module raises at import, and every call raises RmsynthError on a non-OK status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librmsynth.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1810_06250_b200.build` (no CPU fallback exists)")
+_lib = C.CDLL(LIB_PATH)
+
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
+IN_LOS_MAJOR, IN_FREQ_MAJOR, OUT_LOS_MAJOR, OUT_PHI_MAJOR = 0, 1, 0, 2
+SCHEME_AUTO, SCHEME_TF32X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS = 0, 1, 3, 4
+
+EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
+           "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_host", "rmsynth_rmsf",
+           "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
+
+
+class Options(C.Structure):
+    _fields_ = [("struct_size", C.c_int), ("scheme", C.c_int), ("lambda0_mode", C.c_int),
+                ("device", C.c_int), ("lambda0_sq", C.c_double)]
+
+
+_dp, _fp, _ip, _vp = C.POINTER(C.c_double), C.c_void_p, C.c_void_p, C.c_void_p
+_lib.rmsynth_plan_create.argtypes = [C.POINTER(_vp), _dp, _dp, C.c_int, _dp, C.c_int, C.POINTER(Options)]
+_lib.rmsynth_plan_destroy.argtypes = [_vp]
+_lib.rmsynth_plan_info.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+_lib.rmsynth_plan_phase_matrix.argtypes = [_vp, _vp, _vp]
+_lib.rmsynth_execute.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _vp]
+_lib.rmsynth_execute_peaks.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
+_lib.rmsynth_execute_host.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip]
+_lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
+_lib.rmsynth_launch_count.argtypes = [C.c_int]
+_lib.rmsynth_launch_count.restype = C.c_longlong
+_lib.rmsynth_strerror.argtypes = [C.c_int]
+for _n in ("rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"):
+    getattr(_lib, _n).restype = C.c_char_p
+
+
+class RmsynthError(RuntimeError):
+    def __init__(self, status: int):
+        self.status = status
+        super().__init__(f"rmsynth status {status} ({_lib.rmsynth_strerror(status).decode()}): "
+                         f"{_lib.rmsynth_last_error().decode()}")
+
+
+def _check(status: int):
+    if status != OK:
+        raise RmsynthError(status)
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor or numpy array (None -> NULL)."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags.c_contiguous
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def rmsynth_version() -> str:
+    return _lib.rmsynth_version().decode()
+
+
+def rmsynth_launch_count(reset: bool = False) -> int:
+    return int(_lib.rmsynth_launch_count(int(reset)))
+
+
+class Plan:
+    """Owns an rmsynth_plan*.  Methods carry the C entry-point names without the prefix."""
+
+    def __init__(self, nu_hz, w, phi, scheme=SCHEME_AUTO, lambda0_mode=0, lambda0_sq=0.0, device=-1):
+        nu = np.ascontiguousarray(nu_hz, dtype=np.float64)
+        ph = np.ascontiguousarray(phi, dtype=np.float64)
+        ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+        if ww is not None and ww.size != nu.size:
+            raise ValueError("w and nu_hz differ in length")
+        opt = Options(C.sizeof(Options), scheme, lambda0_mode, device, lambda0_sq)
+        self._h = _vp()
+        _check(_lib.rmsynth_plan_create(C.byref(self._h), _d(nu), _d(ww), nu.size, _d(ph), ph.size, C.byref(opt)))
+        K, l0 = C.c_double(), C.c_double()
+        nc, npz, sc = C.c_int(), C.c_int(), C.c_int()
+        _check(_lib.rmsynth_plan_info(self._h, C.byref(l0), C.byref(K), C.byref(nc), C.byref(npz), C.byref(sc)))
+        self.K, self.lambda0_sq, self.n_chan, self.n_phi, self.scheme = K.value, l0.value, nc.value, npz.value, sc.value
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            _lib.rmsynth_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def phase_matrix(self):
+        c = np.empty((self.n_chan, self.n_phi), dtype=np.float32)
+        s = np.empty_like(c)
+        _check(_lib.rmsynth_plan_phase_matrix(self._h, c.ctypes.data, s.ctypes.data))
+        return c, s
+
+    def rmsf(self, phi_eval=None):
+        ph = None if phi_eval is None else np.ascontiguousarray(phi_eval, dtype=np.float64)
+        n = self.n_phi if ph is None else ph.size
+        re, im = np.empty(n), np.empty(n)
+        _check(_lib.rmsynth_rmsf(self._h, _d(ph), n, _d(re), _d(im)))
+        return re + 1j * im
+
+    def execute(self, Q, U, n_pix, layout, FQ, FU, stream=None):
+        """Q,U,FQ,FU: CUDA float32 tensors (contiguous). stream: int cudaStream_t or None."""
+        _check(_lib.rmsynth_execute(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU), stream))
+
+    def execute_peaks(self, Q, U, n_pix, layout, FQ=None, FU=None, peak_amp=None, peak_phi=None,
+                      pa_lambda0=None, pa_zero=None, peak_index=None, stream=None):
+        _check(_lib.rmsynth_execute_peaks(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
+                                          _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
+                                          _ptr(peak_index), stream))
+
+    def execute_host(self, Q, U, n_pix, layout, FQ=None, FU=None, peak_amp=None, peak_phi=None,
+                     pa_lambda0=None, pa_zero=None, peak_index=None):
+        """All arrays in HOST memory (numpy or CPU torch tensors, ideally pinned)."""
+        _check(_lib.rmsynth_execute_host(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
+                                         _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
+                                         _ptr(peak_index)))

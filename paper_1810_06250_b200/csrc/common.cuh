@@ -1,0 +1,94 @@
+// Internal declarations shared by the translation units of librmsynth.so.
+// Nothing here is visible across the C-ABI (include/rmsynth.h is the boundary).
+#pragma once
+#include <cuda_runtime.h>
+#include <atomic>
+#include <mutex>
+#include <string>
+#include <vector>
+#include "rmsynth.h"
+
+namespace rms {
+
+void set_error(const std::string& s);
+rmsynth_status fail(rmsynth_status st, const std::string& s);
+extern std::atomic<long long> g_launches;
+inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+#define RMS_CUDA(expr)                                                                   \
+    do {                                                                                 \
+        cudaError_t e__ = (expr);                                                        \
+        if (e__ != cudaSuccess)                                                          \
+            return rms::fail(e__ == cudaErrorMemoryAllocation ? RMSYNTH_ENOMEM : RMSYNTH_ECUDA, \
+                             std::string(#expr) + ": " + cudaGetErrorString(e__));       \
+    } while (0)
+
+#define RMS_LAUNCH_CHECK(name)                                                           \
+    do {                                                                                 \
+        rms::count_launch();                                                             \
+        cudaError_t e__ = cudaGetLastError();                                            \
+        if (e__ != cudaSuccess)                                                          \
+            return rms::fail(RMSYNTH_ECUDA, std::string(name) + " launch: " + cudaGetErrorString(e__)); \
+    } while (0)
+
+// Tensor-path operand geometry chosen at plan time (see tc_gemm.cu).
+struct TcGeom {
+    int n_tile = 0;      // phi columns per tile (n); UMMA N = 2n
+    int n_phi_tiles = 0; // ceil(n_phi / n)
+    int k_pad = 0;       // n_chan rounded up to the K block
+    int kb = 0;          // channels per K block
+};
+
+}  // namespace rms
+
+struct rmsynth_plan {
+    int n_chan = 0, n_phi = 0, scheme = 0, device = 0, lambda0_mode = 0, sm_count = 0;
+    double K = 0.0, lambda0_sq = 0.0;
+    std::vector<double> lam2, w, phi;     // host copies
+    std::vector<double> R_re, R_im;       // R(phi) on the plan grid (Eq. 12)
+    // device, FP64 plan inputs
+    double* d_delta = nullptr;            // lambda_i^2 - lambda_0^2          [n_chan]
+    double* d_kw = nullptr;               // K w_i                            [n_chan]
+    double* d_phi = nullptr;              //                                  [n_phi]
+    // device, FP32 phase matrix  K w_i cos/sin(th_ik), row i, column k, pitch ldb
+    int ldb = 0;
+    float* d_cos = nullptr;
+    float* d_sin = nullptr;
+    // device, FP32 helpers
+    float* d_phif = nullptr;              // phi as float                     [n_phi]
+    float* d_kwf = nullptr;               // K w_i as float                   [n_chan]
+    float2* d_dpi = nullptr;              // (2/pi)(lambda_i^2-lambda_0^2) as hi+lo floats [n_chan]
+    float2* d_phi2 = nullptr;             // phi as hi+lo floats              [n_phi]
+    // tensor path (tc_gemm.cu)
+    rms::TcGeom tc;
+    float* d_tcB = nullptr;               // pre-split, tiled B operand
+    void* tc_maps = nullptr;              // host-side CUtensorMap cache
+    // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
+    mutable std::mutex mu;
+    static constexpr int kScratch = 12;   // 0-3, 4-7: host-stream slots (Q,U,FQ,FU); 8,9: their maps; 10,11: maps-only cubes
+    mutable float* scratch[kScratch] = {};
+    mutable size_t scratch_bytes[kScratch] = {};
+    mutable cudaStream_t hs[2] = {nullptr, nullptr};
+};
+
+namespace rms {
+
+rmsynth_status ensure_scratch(const rmsynth_plan* p, int slot, size_t bytes, float** out);
+
+// fp32_kernels.cu
+rmsynth_status fp32_table_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
+                                  int layout, float* FQ, float* FU, cudaStream_t st);
+rmsynth_status fp32_sincos_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
+                                   int layout, float* FQ, float* FU, cudaStream_t st);
+// peaks.cu
+rmsynth_status peaks_from_cubes(const rmsynth_plan* p, const float* FQ, const float* FU, long long n_pix,
+                                int out_layout, float* amp, float* phi, float* pa0, float* paz, int* idx,
+                                cudaStream_t st);
+// tc_gemm.cu
+rmsynth_status tc_plan_init(rmsynth_plan* p);
+void tc_plan_free(rmsynth_plan* p);
+rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
+                          float* FQ, float* FU, float* amp, float* phi, float* pa0, float* paz, int* idx,
+                          cudaStream_t st);
+
+}  // namespace rms

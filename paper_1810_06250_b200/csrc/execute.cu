@@ -1,0 +1,130 @@
+// rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_host: argument checks, scheme
+// dispatch (rows a4-a9) and the host-streaming loop (the paper's "each datum crosses the bus
+// once" rule, with pixel chunks instead of LOS batches sized from GPU memory P:L210).
+#include "common.cuh"
+
+namespace rms {
+
+static rmsynth_status check_args(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
+                                 int layout, bool need_cubes, const float* FQ, const float* FU) {
+    if (!p) return fail(RMSYNTH_EINVAL, "plan is NULL");
+    if (n_pix < 0) return fail(RMSYNTH_EINVAL, "n_pix < 0");
+    if (layout & ~3) return fail(RMSYNTH_EINVAL, "unknown layout flags");
+    if (n_pix == 0) return RMSYNTH_OK;
+    if (!Q || !U) return fail(RMSYNTH_EINVAL, "Q/U is NULL");
+    if ((FQ == nullptr) != (FU == nullptr)) return fail(RMSYNTH_EINVAL, "FQ and FU must both be given or both NULL");
+    if (need_cubes && !FQ) return fail(RMSYNTH_EINVAL, "FQ/FU is NULL");
+    if (n_pix > (1LL << 40)) return fail(RMSYNTH_EINVAL, "n_pix too large");
+    return RMSYNTH_OK;
+}
+
+// Device-resident contraction + optional maps on one stream; never synchronises.
+static rmsynth_status run_device(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
+                                 float* FQ, float* FU, float* amp, float* phi, float* pa0, float* paz, int* idx,
+                                 cudaStream_t st) {
+    const bool want_maps = amp || phi || pa0 || paz || idx;
+    if (p->scheme == RMSYNTH_SCHEME_TF32X3)
+        return tc_execute(p, Q, U, n_pix, layout, FQ, FU, amp, phi, pa0, paz, idx, st);
+    // FP32 CUDA-core comparison paths: cubes first, then the stand-alone peak kernel.
+    if (!FQ) {
+        std::lock_guard<std::mutex> g(p->mu);
+        size_t bytes = sizeof(float) * (size_t)n_pix * p->n_phi;
+        rmsynth_status s;
+        if ((s = ensure_scratch(p, 10, bytes, &FQ)) || (s = ensure_scratch(p, 11, bytes, &FU))) return s;
+    }
+    rmsynth_status s = p->scheme == RMSYNTH_SCHEME_FP32_TABLE
+                           ? fp32_table_execute(p, Q, U, n_pix, layout, FQ, FU, st)
+                           : fp32_sincos_execute(p, Q, U, n_pix, layout, FQ, FU, st);
+    if (s != RMSYNTH_OK || !want_maps) return s;
+    return peaks_from_cubes(p, FQ, FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, amp, phi, pa0, paz, idx, st);
+}
+
+}  // namespace rms
+
+using namespace rms;
+
+extern "C" {
+
+rmsynth_status rmsynth_execute(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
+                               int layout, float* FQ, float* FU, void* stream) {
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, true, FQ, FU);
+    if (s != RMSYNTH_OK || n_pix == 0) return s;
+    return run_device(plan, Q, U, n_pix, layout, FQ, FU, nullptr, nullptr, nullptr, nullptr, nullptr,
+                      (cudaStream_t)stream);
+}
+
+rmsynth_status rmsynth_execute_peaks(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
+                                     int layout, float* FQ, float* FU, float* peak_amp, float* peak_phi,
+                                     float* pa_lambda0, float* pa_zero, int* peak_index, void* stream) {
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, FQ, FU);
+    if (s != RMSYNTH_OK || n_pix == 0) return s;
+    if (!FQ && !(peak_amp || peak_phi || pa_lambda0 || pa_zero || peak_index))
+        return fail(RMSYNTH_EINVAL, "no output requested");
+    return run_device(plan, Q, U, n_pix, layout, FQ, FU, peak_amp, peak_phi, pa_lambda0, pa_zero, peak_index,
+                      (cudaStream_t)stream);
+}
+
+rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
+                                    int layout, float* FQ, float* FU, float* peak_amp, float* peak_phi,
+                                    float* pa_lambda0, float* pa_zero, int* peak_index) {
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, FQ, FU);
+    if (s != RMSYNTH_OK || n_pix == 0) return s;
+    const rmsynth_plan* p = plan;
+    const bool want_maps = peak_amp || peak_phi || pa_lambda0 || pa_zero || peak_index;
+    if (!FQ && !want_maps) return fail(RMSYNTH_EINVAL, "no output requested");
+    RMS_CUDA(cudaSetDevice(p->device));
+    std::lock_guard<std::mutex> g(p->mu);
+    const int nc = p->n_chan, np = p->n_phi;
+    const bool in_freq = layout & RMSYNTH_IN_FREQ_MAJOR, out_phi = layout & RMSYNTH_OUT_PHI_MAJOR;
+    // ~256 MB of device buffers per slot, two slots in flight
+    long long chunk = (256LL << 20) / (8LL * (nc + np));
+    chunk = chunk / 1024 * 1024;
+    if (chunk < 1024) chunk = 1024;
+    if (chunk > n_pix) chunk = n_pix;
+    float *dQ[2], *dU[2], *dFQ[2], *dFU[2], *dM[2];
+    for (int b = 0; b < 2; ++b) {
+        if (!p->hs[b]) RMS_CUDA(cudaStreamCreateWithFlags(&p->hs[b], cudaStreamNonBlocking));
+        if ((s = ensure_scratch(p, 4 * b + 0, sizeof(float) * chunk * nc, &dQ[b])) ||
+            (s = ensure_scratch(p, 4 * b + 1, sizeof(float) * chunk * nc, &dU[b])) ||
+            (s = ensure_scratch(p, 4 * b + 2, sizeof(float) * chunk * np, &dFQ[b])) ||
+            (s = ensure_scratch(p, 4 * b + 3, sizeof(float) * chunk * np, &dFU[b])) ||
+            (s = ensure_scratch(p, 8 + b, sizeof(float) * chunk * 5, &dM[b])))
+            return s;
+    }
+    int it = 0;
+    for (long long p0 = 0; p0 < n_pix; p0 += chunk, ++it) {
+        const int b = it & 1;
+        const long long n = n_pix - p0 < chunk ? n_pix - p0 : chunk;
+        cudaStream_t st = p->hs[b];
+        if (in_freq) {   // columns [p0, p0+n) of [chan][pix] -> compact [chan][n]
+            RMS_CUDA(cudaMemcpy2DAsync(dQ[b], n * 4, Q + p0, n_pix * 4, n * 4, nc, cudaMemcpyHostToDevice, st));
+            RMS_CUDA(cudaMemcpy2DAsync(dU[b], n * 4, U + p0, n_pix * 4, n * 4, nc, cudaMemcpyHostToDevice, st));
+        } else {
+            RMS_CUDA(cudaMemcpyAsync(dQ[b], Q + p0 * nc, sizeof(float) * n * nc, cudaMemcpyHostToDevice, st));
+            RMS_CUDA(cudaMemcpyAsync(dU[b], U + p0 * nc, sizeof(float) * n * nc, cudaMemcpyHostToDevice, st));
+        }
+        float* m = dM[b];
+        s = run_device(p, dQ[b], dU[b], n, layout, dFQ[b], dFU[b], peak_amp ? m : nullptr,
+                       peak_phi ? m + chunk : nullptr, pa_lambda0 ? m + 2 * chunk : nullptr,
+                       pa_zero ? m + 3 * chunk : nullptr, peak_index ? (int*)(m + 4 * chunk) : nullptr, st);
+        if (s != RMSYNTH_OK) return s;
+        if (FQ) {
+            if (out_phi) {
+                RMS_CUDA(cudaMemcpy2DAsync(FQ + p0, n_pix * 4, dFQ[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, st));
+                RMS_CUDA(cudaMemcpy2DAsync(FU + p0, n_pix * 4, dFU[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, st));
+            } else {
+                RMS_CUDA(cudaMemcpyAsync(FQ + p0 * np, dFQ[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, st));
+                RMS_CUDA(cudaMemcpyAsync(FU + p0 * np, dFU[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, st));
+            }
+        }
+        float* outs[5] = {peak_amp, peak_phi, pa_lambda0, pa_zero, (float*)peak_index};
+        for (int j = 0; j < 5; ++j)
+            if (outs[j])
+                RMS_CUDA(cudaMemcpyAsync(outs[j] + p0, m + j * chunk, sizeof(float) * n, cudaMemcpyDeviceToHost, st));
+    }
+    RMS_CUDA(cudaStreamSynchronize(p->hs[0]));
+    RMS_CUDA(cudaStreamSynchronize(p->hs[1]));
+    return RMSYNTH_OK;
+}
+
+}  // extern "C"

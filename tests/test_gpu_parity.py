@@ -1,0 +1,253 @@
+"""GPU parity tests proper: every call goes through the C-ABI binding and is compared with
+the FP64 oracle on the same seeded inputs (run with `-m gpu` on a B200)."""
+import numpy as np
+import pytest
+import torch
+
+import rmsynth_inputs as ri
+from parity import TOL, check_cubes, check_peaks, oracle_reference
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def b():
+    assert torch.cuda.is_available(), "gpu tests need a B200"
+    from paper_1810_06250_b200 import binding
+    return binding
+
+
+def scheme_ids(b):
+    return {"tf32x3": b.SCHEME_TF32X3, "fp32_table": b.SCHEME_FP32_TABLE, "fp32_sincos": b.SCHEME_FP32_SINCOS}
+
+
+SCHEMES = ["tf32x3", "fp32_table", "fp32_sincos"]
+LAYOUTS = [("los", "los"), ("los", "phi"), ("freq", "los"), ("freq", "phi")]
+
+
+def run_gpu(b, plan, q_los, u_los, lin, lout, peaks=False, cubes=True, host=False):
+    """q_los/u_los: host float32 [n_pix, n_chan].  Returns LOS-major numpy outputs."""
+    n_pix, n_chan = q_los.shape
+    n_phi = plan.n_phi
+    layout = (b.IN_FREQ_MAJOR if lin == "freq" else 0) | (b.OUT_PHI_MAJOR if lout == "phi" else 0)
+    dev = "cpu" if host else "cuda"
+    q = torch.from_numpy(q_los if lin == "los" else np.ascontiguousarray(q_los.T)).to(dev)
+    u = torch.from_numpy(u_los if lin == "los" else np.ascontiguousarray(u_los.T)).to(dev)
+    shape = (n_pix, n_phi) if lout == "los" else (n_phi, n_pix)
+    FQ = torch.full(shape, float("nan"), dtype=torch.float32, device=dev) if cubes else None
+    FU = torch.full(shape, float("nan"), dtype=torch.float32, device=dev) if cubes else None
+    maps = {}
+    if peaks:
+        for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+            maps[k] = torch.full((n_pix,), float("nan"), dtype=torch.float32, device=dev)
+        maps["peak_index"] = torch.full((n_pix,), -1, dtype=torch.int32, device=dev)
+    if host:
+        plan.execute_host(q, u, n_pix, layout, FQ, FU, **maps)
+    elif peaks:
+        plan.execute_peaks(q, u, n_pix, layout, FQ, FU, **maps)
+        torch.cuda.synchronize()
+    else:
+        plan.execute(q, u, n_pix, layout, FQ, FU)
+        torch.cuda.synchronize()
+    out = {}
+    if cubes:
+        out["FQ"] = FQ.cpu().numpy() if lout == "los" else FQ.cpu().numpy().T
+        out["FU"] = FU.cpu().numpy() if lout == "los" else FU.cpu().numpy().T
+    if peaks:
+        out["maps"] = {("kstar" if k == "peak_index" else k): v.cpu().numpy() for k, v in maps.items()}
+    return out
+
+
+def inputs(cfg_id, n_pix, start=0):
+    cfg = ri.CONFIGS[cfg_id]
+    nu, w, phi = ri.grids(cfg)
+    q, u = ri.generate_pixels(cfg, torch.arange(start, start + n_pix))
+    return cfg, nu, w, phi, q.numpy(), u.numpy()
+
+
+# ------------------------------------------------------------------ plan (rows a1-a3)
+@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4, 5])
+def test_plan_scalars_phase_matrix_and_rmsf(b, oracle_mod, cfg_id):
+    cfg = ri.CONFIGS[cfg_id]
+    nu, w, phi = ri.grids(cfg)
+    for mode, l0 in ((0, 0.0), (1, 0.0), (2, 0.0), (2, 1.25)):
+        op = oracle_mod.make_plan(nu, w, phi, mode, l0)
+        gp = b.Plan(nu, w, phi, scheme=b.SCHEME_FP32_TABLE, lambda0_mode=mode, lambda0_sq=l0)
+        assert abs(gp.K - op.K) <= 1e-15 * op.K and abs(gp.lambda0_sq - op.lambda0_sq) <= 1e-14 * max(op.lambda0_sq, 1)
+        R = gp.rmsf()
+        assert np.max(np.abs(R - oracle_mod.rmsf(op))) < 1e-11
+        pe = np.linspace(phi[0] * 1.5, phi[-1] * 1.5, 77) + 0.123
+        assert np.max(np.abs(gp.rmsf(pe) - oracle_mod.rmsf(op, pe))) < 1e-11
+        if mode == 0:
+            c, s = gp.phase_matrix()
+            th = 2.0 * phi[None, :] * (op.lam2 - op.lambda0_sq)[:, None]
+            kw = (op.K * op.w)[:, None]
+            scale = float(kw.max())
+            assert np.max(np.abs(c - kw * np.cos(th))) <= 1.2e-7 * scale
+            assert np.max(np.abs(s - kw * np.sin(th))) <= 1.2e-7 * scale
+        gp.destroy()
+
+
+# ------------------------------------------------------------------ cubes (rows a4-a6, a9)
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("lin,lout", LAYOUTS)
+@pytest.mark.parametrize("cfg_id,n_pix", [(1, 301), (2, 257), (3, 130), (4, 200), (5, 1031)])
+def test_cubes_match_oracle(b, oracle_mod, scheme, lin, lout, cfg_id, n_pix):
+    """Every config's grids at a pixel count spanning several tiles plus a ragged tail, all four
+    layout combinations (reading A7)."""
+    cfg, nu, w, phi, q, u = inputs(cfg_id, n_pix, start=7)
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, lin, lout)
+    worst = check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} cfg{cfg_id} {lin}->{lout}")
+    print(f"{scheme} cfg{cfg_id} {lin}->{lout}: max err/T_p = {worst:.2e}")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_full_config1_cube(b, oracle_mod, scheme):
+    """BASELINE.json configs[0] in full: 64x64 pixels, LOS-major in and out."""
+    cfg = ri.CONFIGS[1]
+    nu, w, phi = ri.grids(cfg)
+    Q, U = ri.generate_cube(cfg, "cpu")
+    q, u = Q.numpy(), U.numpy()
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, "los", "los")
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} full config 1")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("n_chan,n_phi,n_pix", [(1, 1, 1), (3, 2, 5), (37, 19, 129), (8, 9, 16), (129, 257, 127),
+                                                (33, 513, 3), (1000, 7, 260)])
+def test_odd_shapes_and_degenerate_sizes(b, oracle_mod, scheme, n_chan, n_phi, n_pix):
+    rng = np.random.default_rng(n_chan * 1000 + n_phi)
+    nu = np.sort(rng.uniform(0.9e9, 1.8e9, n_chan))
+    w = rng.uniform(0.0, 1.0, n_chan)
+    w[0] = 0.7
+    phi = np.sort(rng.uniform(-300, 300, n_phi))            # non-uniform, unsorted grids are legal
+    q = rng.standard_normal((n_pix, n_chan)).astype(np.float32)
+    u = rng.standard_normal((n_pix, n_chan)).astype(np.float32)
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    for lin, lout in LAYOUTS:
+        out = run_gpu(b, plan, q, u, lin, lout)
+        check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} {n_chan}x{n_phi}x{n_pix} {lin}->{lout}")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_coherent_worst_case_and_dynamic_range(b, oracle_mod, scheme):
+    """All channels in phase at an on-grid depth (partial sums grow to the full norm: the worst
+    case for accumulator rounding), plus pixels scaled by 1e-20 .. 1e+20."""
+    cfg = ri.CONFIGS[4]
+    nu, w, phi = ri.grids(cfg)
+    lam2 = (ri.C_M_PER_S / nu) ** 2
+    n_pix = 140
+    rng = np.random.default_rng(11)
+    phi0 = phi[rng.integers(0, phi.size, n_pix)]
+    chi = rng.uniform(0, np.pi, n_pix)
+    P = np.exp(2j * (chi[:, None] + phi0[:, None] * lam2[None, :]))
+    scale = 10.0 ** rng.integers(-20, 21, n_pix)
+    scale[:8] = 1.0
+    q = (P.real * scale[:, None]).astype(np.float32)
+    u = (P.imag * scale[:, None]).astype(np.float32)
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, "freq", "phi")
+    worst = check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} coherent")
+    print(f"{scheme} coherent worst case: max err/T_p = {worst:.2e}")
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ peak maps (row a7)
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("lin,lout", [("freq", "phi"), ("los", "los")])
+@pytest.mark.parametrize("cfg_id,n_pix", [(4, 300), (5, 517), (1, 200)])
+def test_peak_maps(b, oracle_mod, scheme, lin, lout, cfg_id, n_pix):
+    cfg, nu, w, phi, q, u = inputs(cfg_id, n_pix)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, lin, lout, peaks=True)
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, "cubes with peaks")
+    nd = check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], cfg.dphi, f"{scheme} cfg{cfg_id}")
+    assert nd <= max(1, n_pix // 50)
+    # maps only (no cubes written)
+    out2 = run_gpu(b, plan, q, u, lin, lout, peaks=True, cubes=False)
+    for k, v in out["maps"].items():
+        assert np.array_equal(v, out2["maps"][k]), k
+    plan.destroy()
+
+
+def test_peak_refinement_on_nonuniform_grid_and_edges(b, oracle_mod):
+    nu = np.linspace(1.0e9, 2.0e9, 64)
+    phi = np.array([-90.0, -60, -45, -20, -5, 0, 12, 30, 55, 80, 120])
+    lam2 = (ri.C_M_PER_S / nu) ** 2
+    phi0 = np.array([-90.0, 120.0, 3.0, -50.0, 41.0, 0.0])
+    P = np.exp(2j * (0.4 + phi0[:, None] * lam2[None, :]))
+    q, u = P.real.astype(np.float32), P.imag.astype(np.float32)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, None, phi, q, u)
+    for scheme in SCHEMES:
+        plan = b.Plan(nu, None, phi, scheme=scheme_ids(b)[scheme])
+        out = run_gpu(b, plan, q, u, "los", "los", peaks=True)
+        check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], 5.0, scheme)
+        assert out["maps"]["kstar"][0] == 0 and out["maps"]["kstar"][1] == phi.size - 1
+        plan.destroy()
+
+
+# ------------------------------------------------------------------ host streaming + API edges
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("lin,lout", [("freq", "phi"), ("los", "los"), ("freq", "los")])
+def test_execute_host_matches_oracle(b, oracle_mod, scheme, lin, lout):
+    cfg, nu, w, phi, q, u = inputs(1, 2500)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, lin, lout, peaks=True, host=True)
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, "execute_host")
+    check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], cfg.dphi, "execute_host")
+    plan.destroy()
+
+
+def test_api_edges(b):
+    nu, phi = np.linspace(1e9, 2e9, 16), np.linspace(-10, 10, 5)
+    for scheme in SCHEMES:
+        plan = b.Plan(nu, None, phi, scheme=scheme_ids(b)[scheme])
+        q = torch.zeros(4, 16, device="cuda")
+        f = torch.zeros(4, 5, device="cuda")
+        plan.execute(None, None, 0, 0, None, None)                 # n_pix = 0: successful no-op
+        for bad in (lambda: plan.execute(q, q, -1, 0, f, f), lambda: plan.execute(q, q, 4, 4, f, f),
+                    lambda: plan.execute(None, q, 4, 0, f, f), lambda: plan.execute(q, q, 4, 0, None, f),
+                    lambda: plan.execute_peaks(q, q, 4, 0)):
+            with pytest.raises(b.RmsynthError) as e:
+                bad()
+            assert e.value.status == b.EINVAL
+        # runs on a caller-provided stream and does not modify its inputs
+        s = torch.cuda.Stream()
+        q.normal_()
+        q0 = q.clone()
+        with torch.cuda.stream(s):
+            plan.execute(q, q, 4, 0, f, f, stream=s.cuda_stream)
+        s.synchronize()
+        assert torch.equal(q, q0) and torch.isfinite(f).all()
+        n0 = b.rmsynth_launch_count(True)
+        plan.execute(q, q, 4, 0, f, f)
+        assert b.rmsynth_launch_count() >= 1 and n0 >= 1
+        plan.destroy()
+
+
+def test_nonfinite_samples_stay_in_their_pixel(b):
+    nu, phi = np.linspace(1e9, 2e9, 40), np.linspace(-100, 100, 21)
+    for scheme in SCHEMES:
+        plan = b.Plan(nu, None, phi, scheme=scheme_ids(b)[scheme])
+        q = torch.randn(300, 40, device="cuda")
+        u = torch.randn(300, 40, device="cuda")
+        q[17, 3] = float("nan")
+        u[150, 39] = float("inf")
+        fq = torch.zeros(300, 21, device="cuda")
+        fu = torch.zeros(300, 21, device="cuda")
+        plan.execute(q, u, 300, 0, fq, fu)
+        torch.cuda.synchronize()
+        bad = ~(torch.isfinite(fq).all(1) & torch.isfinite(fu).all(1))
+        assert sorted(torch.nonzero(bad).flatten().tolist()) == [17, 150], scheme
+        plan.destroy()
