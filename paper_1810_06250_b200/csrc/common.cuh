@@ -65,7 +65,7 @@ struct rmsynth_plan {
     void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
-    static constexpr int kScratch = 12;   // 0-3, 4-7: host-stream slots (Q,U,FQ,FU); 8,9: their maps; 10,11: maps-only cubes
+    static constexpr int kScratch = 14;   // 0-7 host-stream slots (Q,U,FQ,FU x2); 8,9 their maps; 10,11 maps-only cubes; 12,13 TMA repack
     mutable float* scratch[kScratch] = {};
     mutable size_t scratch_bytes[kScratch] = {};
     mutable cudaStream_t hs[2] = {nullptr, nullptr};
