@@ -67,6 +67,11 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
         "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
@@ -160,6 +165,8 @@ struct TcParams {
     int n_stages;        // ceil(n_chan / KS)
     int n_pix_tiles;
     int out_phi_major;   // 1: F[k*n_pix+p], 0: F[p*n_phi+k]
+    int a3d;             // frequency-major input addressed through a 3-D map (32 pix, chan, pix/32)
+    int n_items;         // n_pix_tiles * n_phi_tiles
     const float* blob;
     float* FQ;
     float* FU;
@@ -208,28 +215,33 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         // ===================== TMA producer =====================
         if (lane == 0) {
             uint32_t st = 0, ph = 0;
-            for (int t = blockIdx.x; t < prm.n_pix_tiles; t += gridDim.x) {
+            // Work items are (pixel tile, depth tile) pairs dealt round-robin, so the CTAs running at
+            // any moment share ~grid/n_phi_tiles pixel tiles: A is fetched from HBM once and re-read from L2.
+            for (int item = blockIdx.x; item < prm.n_items; item += gridDim.x) {
+                const int t = item / prm.n_phi_tiles, j = item - t * prm.n_phi_tiles;
                 const int pix0 = t * TC_M;
-                for (int j = 0; j < prm.n_phi_tiles; ++j) {
-                    const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) +
-                                          (size_t)j * prm.n_stages * 2 * b_part_bytes;
-                    for (int s = 0; s < prm.n_stages; ++s) {
-                        mbar_wait(&empty[st], ph ^ 1);
-                        mbar_expect_tx(&full[st], stage_tx);
-                        const uint32_t sb = smem_base + st * Cfg::kStageBytes;
-                        if (IN_MN) {   // [chan][pix]: four boxes of 32 pixels x KS channels per operand
+                const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) + (size_t)j * prm.n_stages * 2 * b_part_bytes;
+                for (int s = 0; s < prm.n_stages; ++s) {
+                    mbar_wait(&empty[st], ph ^ 1);
+                    mbar_expect_tx(&full[st], stage_tx);
+                    const uint32_t sb = smem_base + st * Cfg::kStageBytes;
+                    if (IN_MN) {
+                        if (prm.a3d) {   // one box: 32 pixels x KS channels x 4 pixel groups
+                            tma_load_3d(sb, &mapQ, 0, s * KS, pix0 / 32, &full[st]);
+                            tma_load_3d(sb + Cfg::kAPart, &mapU, 0, s * KS, pix0 / 32, &full[st]);
+                        } else {         // four boxes of 32 pixels x KS channels per operand
 #pragma unroll
                             for (int g = 0; g < 4; ++g) {
                                 tma_load_2d(sb + g * (KS * 128), &mapQ, pix0 + 32 * g, s * KS, &full[st]);
                                 tma_load_2d(sb + Cfg::kAPart + g * (KS * 128), &mapU, pix0 + 32 * g, s * KS, &full[st]);
                             }
-                        } else {       // [pix][chan]: one box of KS channels x 128 pixels per operand
-                            tma_load_2d(sb, &mapQ, s * KS, pix0, &full[st]);
-                            tma_load_2d(sb + Cfg::kAPart, &mapU, s * KS, pix0, &full[st]);
                         }
-                        bulk_load(sb + 4 * Cfg::kAPart, bsrc + (size_t)s * 2 * b_part_bytes, 2 * b_part_bytes, &full[st]);
-                        if (++st == S) { st = 0; ph ^= 1; }
+                    } else {             // [pix][chan]: one box of KS channels x 128 pixels per operand
+                        tma_load_2d(sb, &mapQ, s * KS, pix0, &full[st]);
+                        tma_load_2d(sb + Cfg::kAPart, &mapU, s * KS, pix0, &full[st]);
                     }
+                    bulk_load(sb + 4 * Cfg::kAPart, bsrc + (size_t)s * 2 * b_part_bytes, 2 * b_part_bytes, &full[st]);
+                    if (++st == S) { st = 0; ph ^= 1; }
                 }
             }
         }
@@ -240,8 +252,7 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)IN_MN << 15) |
                                    ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
             uint32_t st = 0, ph = 0, ab = 0, aph = 0;
-            for (int t = blockIdx.x; t < prm.n_pix_tiles; t += gridDim.x)
-                for (int j = 0; j < prm.n_phi_tiles; ++j)
+            for (int item = blockIdx.x; item < prm.n_items; item += gridDim.x)
                     for (int c = 0; c < n_chunks; ++c) {
                         mbar_wait(&acc_empty[ab], aph ^ 1);
                         tc_fence_after();
@@ -285,8 +296,7 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
         const int tt = threadIdx.x - 128;   // 0..127
         uint32_t st = 0, ph = 0;
-        const long long total = (long long)((prm.n_pix_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) *
-                                prm.n_phi_tiles * prm.n_stages;
+        const long long total = (long long)((prm.n_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * prm.n_stages;
         for (long long it = 0; it < total; ++it) {
             mbar_wait(&full[st], ph);
             uint8_t* sg = smem_gen + (size_t)st * Cfg::kStageBytes;
@@ -314,9 +324,10 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         uint32_t ab = 0, aph = 0;
         float acc[128];
-        for (int t = blockIdx.x; t < prm.n_pix_tiles; t += gridDim.x) {
+        for (int item = blockIdx.x; item < prm.n_items; item += gridDim.x) {
+            const int t = item / prm.n_phi_tiles, j = item - t * prm.n_phi_tiles;
             const long long p = (long long)t * TC_M + q * 32 + lane;
-            for (int j = 0; j < prm.n_phi_tiles; ++j) {
+            {
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&acc_full[ab], aph);
                     tc_fence_after();
@@ -414,6 +425,19 @@ __global__ void tc_repack_kernel(const float* __restrict__ src, float* __restric
     dst[i] = c < cols ? src[r * cols + c] : 0.f;
 }
 
+static rmsynth_status make_map3(CUtensorMap* m, const float* base, uint64_t n_chan, uint64_t n_pix, uint64_t pitch_floats,
+                                uint32_t ks) {
+    cuuint64_t dims[3] = {32, n_chan, n_pix / 32};
+    cuuint64_t strides[2] = {pitch_floats * 4, 128};
+    cuuint32_t box[3] = {32, ks, 4};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = get_encode_fn()(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides, box, es,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(RMSYNTH_ECUDA, "cuTensorMapEncodeTiled(3d) failed with code " + std::to_string((int)r));
+    return RMSYNTH_OK;
+}
+
 static rmsynth_status make_map(CUtensorMap* m, const float* base, uint64_t inner, uint64_t outer, uint64_t pitch_floats,
                                uint32_t box_in, uint32_t box_out, CUtensorMapSwizzle sw) {
     cuuint64_t dims[2] = {inner, outer};
@@ -458,7 +482,11 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
         U = u2;
     }
     CUtensorMap mq, mu_;
-    if (in_freq) {
+    const bool a3d = in_freq && (n_pix % 32 == 0);
+    if (a3d) {
+        if ((s = make_map3(&mq, Q, p->n_chan, n_pix, pitch, TC_KS)) || (s = make_map3(&mu_, U, p->n_chan, n_pix, pitch, TC_KS)))
+            return s;
+    } else if (in_freq) {
         if ((s = make_map(&mq, Q, n_pix, p->n_chan, pitch, 32, TC_KS, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)) ||
             (s = make_map(&mu_, U, n_pix, p->n_chan, pitch, 32, TC_KS, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)))
             return s;
@@ -478,10 +506,12 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     prm.n_stages = p->tc.k_pad / TC_KS;
     prm.n_pix_tiles = (int)((n_pix + TC_M - 1) / TC_M);
     prm.out_phi_major = out_phi ? 1 : 0;
+    prm.a3d = a3d ? 1 : 0;
+    prm.n_items = prm.n_pix_tiles * prm.n_phi_tiles;
     prm.blob = p->d_tcB;
     prm.FQ = FQ;
     prm.FU = FU;
-    const int grid = prm.n_pix_tiles < p->sm_count ? prm.n_pix_tiles : p->sm_count;
+    const int grid = prm.n_items < p->sm_count ? prm.n_items : p->sm_count;
     if (in_freq)
         tc_rmsynth_kernel<TC_KS, 1><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
     else
