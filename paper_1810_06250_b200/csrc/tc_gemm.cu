@@ -21,6 +21,8 @@
 // (SWIZZLE_128B_ATOM_32B TMA boxes, UMMA layout SWIZZLE_128B_BASE32B): no transpose pass exists.
 #include <cuda.h>
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 #include "common.cuh"
 
 namespace rms {
@@ -95,6 +97,9 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
           "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
         : "r"(taddr));
 }
+__device__ __forceinline__ void st_global_pred(unsigned long long addr, float v, bool pred) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %2, 0;\n@p st.global.f32 [%0], %1;\n}" ::"l"(addr), "f"(v), "r"((int)pred) : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -167,6 +172,7 @@ struct TcParams {
     int out_phi_major;   // 1: F[k*n_pix+p], 0: F[p*n_phi+k]
     int a3d;             // frequency-major input addressed through a 3-D map (32 pix, chan, pix/32)
     int n_items;         // n_pix_tiles * n_phi_tiles
+    long long* prof;     // debug (RMSYNTH_TC_PROFILE=1): per-CTA cycles the MMA thread waited on {full, ready, acc_empty}, total
     const float* blob;
     float* FQ;
     float* FU;
@@ -252,16 +258,23 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)IN_MN << 15) |
                                    ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
             uint32_t st = 0, ph = 0, ab = 0, aph = 0;
+            long long w_full = 0, w_ready = 0, w_acc = 0, t_begin = clock64(), t0 = 0;
+            const bool prof = prm.prof != nullptr;
             for (int item = blockIdx.x; item < prm.n_items; item += gridDim.x)
                     for (int c = 0; c < n_chunks; ++c) {
+                        if (prof) t0 = clock64();
                         mbar_wait(&acc_empty[ab], aph ^ 1);
+                        if (prof) w_acc += clock64() - t0;
                         tc_fence_after();
                         const uint32_t d_tmem = tmem + ab * 256;
                         const int s_end = min(prm.n_stages, (c + 1) * Cfg::kStagesPerChunk);
                         uint32_t first = 1;
                         for (int s = c * Cfg::kStagesPerChunk; s < s_end; ++s) {
+                            if (prof) t0 = clock64();
                             mbar_wait(&full[st], ph);
+                            if (prof) { long long t1 = clock64(); w_full += t1 - t0; t0 = t1; }
                             mbar_wait(&ready[st], ph);
+                            if (prof) w_ready += clock64() - t0;
                             tc_fence_after();
                             const uint32_t sb = smem_base + st * Cfg::kStageBytes;
                             const uint32_t aQ = sb, aU = sb + Cfg::kAPart, aQl = sb + 2 * Cfg::kAPart, aUl = sb + 3 * Cfg::kAPart;
@@ -288,6 +301,10 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                         umma_commit(&acc_full[ab]);
                         if (++ab == 2) { ab = 0; aph ^= 1; }
                     }
+            if (prof) {
+                prm.prof[blockIdx.x * 4 + 0] = w_full; prm.prof[blockIdx.x * 4 + 1] = w_ready;
+                prm.prof[blockIdx.x * 4 + 2] = w_acc;  prm.prof[blockIdx.x * 4 + 3] = clock64() - t_begin;
+            }
         }
         __syncwarp();
       }
@@ -351,17 +368,26 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
                 if (p < prm.n_pix) {
+                    // my columns cbase..cbase+127 of [FQ(0..n) | FU(n..2n)]; nv depths of this tile are real.
+                    // All bounds are warp-uniform; addresses are base + i*stride with compile-time i.
+                    const int nv = min(n, prm.n_phi - j * n);
+                    const int q_end = nv - cbase, u_beg = n - cbase, u_end = n + nv - cbase;
+                    const long long sb = prm.out_phi_major ? 4LL * prm.n_pix : 4LL;   // byte stride between depths
+                    const long long kq = (long long)j * n + cbase, ku = kq - n;
+                    unsigned long long aq = (unsigned long long)(prm.FQ + (prm.out_phi_major ? kq * prm.n_pix + p : p * prm.n_phi + kq));
+                    unsigned long long au = (unsigned long long)(prm.FU + (prm.out_phi_major ? ku * prm.n_pix + p : p * prm.n_phi + ku));
+                    asm volatile("" : "+l"(aq), "+l"(au));   // keep the bases in registers (no rematerialisation)
 #pragma unroll
-                    for (int i = 0; i < 128; ++i) {
-                        const int col = cbase + i;
-                        if (col < N2) {
-                            const bool is_u = col >= n;
-                            const int k = j * n + (is_u ? col - n : col);
-                            if (k < prm.n_phi) {
-                                float* dst = is_u ? prm.FU : prm.FQ;
-                                const size_t off = prm.out_phi_major ? (size_t)k * prm.n_pix + p : (size_t)p * prm.n_phi + k;
-                                dst[off] = acc[i];
-                            }
+                    for (int g = 0; g < 4; ++g) {
+                        if (g * 32 < q_end) {              // warp-uniform
+#pragma unroll
+                            for (int i = g * 32; i < g * 32 + 32; ++i)
+                                st_global_pred(aq + i * sb, acc[i], i < q_end);
+                        }
+                        if (g * 32 + 32 > u_beg && g * 32 < u_end) {
+#pragma unroll
+                            for (int i = g * 32; i < g * 32 + 32; ++i)
+                                st_global_pred(au + i * sb, acc[i], (unsigned)(i - u_beg) < (unsigned)nv);
                         }
                     }
                 }
@@ -512,11 +538,25 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     prm.FQ = FQ;
     prm.FU = FU;
     const int grid = prm.n_items < p->sm_count ? prm.n_items : p->sm_count;
+    prm.prof = nullptr;
+    static const bool want_prof = getenv("RMSYNTH_TC_PROFILE") != nullptr;
+    if (want_prof) {
+        RMS_CUDA(cudaMalloc(&prm.prof, sizeof(long long) * 4 * grid));
+    }
     if (in_freq)
         tc_rmsynth_kernel<TC_KS, 1><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
     else
         tc_rmsynth_kernel<TC_KS, 0><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
     RMS_LAUNCH_CHECK("tc_rmsynth_kernel");
+    if (want_prof) {   // debug only: synchronises
+        std::vector<long long> h(4 * grid);
+        RMS_CUDA(cudaMemcpy(h.data(), prm.prof, sizeof(long long) * 4 * grid, cudaMemcpyDeviceToHost));
+        cudaFree(prm.prof);
+        double a[4] = {0, 0, 0, 0};
+        for (int i = 0; i < grid; ++i) for (int j = 0; j < 4; ++j) a[j] += (double)h[4 * i + j] / grid;
+        fprintf(stderr, "[rmsynth tc profile] MMA thread: total %.0f cyc; waiting full %.1f%% ready %.1f%% acc_empty %.1f%%\n",
+                a[3], 100 * a[0] / a[3], 100 * a[1] / a[3], 100 * a[2] / a[3]);
+    }
     if (!want_maps) return RMSYNTH_OK;
     return peaks_from_cubes(p, FQ, FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, amp, phi, pa0, paz, idx, st);
 }
