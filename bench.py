@@ -50,17 +50,21 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
                                           "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
-            threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True).start()
+            threading.Thread(target=lambda: [self.lines.append((time.time(), l)) for l in self.proc.stdout], daemon=True).start()
         except OSError:
             self.proc = None
 
-    def stop(self):
+    def stop(self, t_begin=0.0, t_end=float("inf")):
+        """Summary over the samples that arrived inside [t_begin, t_end] (the timed region)."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        time.sleep(0.12)
         self.proc.terminate()
         sm, mx, reasons = [], [], set()
-        for l in self.lines:
+        inside = [l for t, l in self.lines if t_begin <= t <= t_end + 0.1]
+        if not inside and self.lines:      # region shorter than the sampling period: nearest sample
+            inside = [min(self.lines, key=lambda tl: abs(tl[0] - 0.5 * (t_begin + t_end)))[1]]
+        for l in inside:
             f = [x.strip() for x in l.split(",")]
             if len(f) < 9:
                 continue
@@ -71,16 +75,15 @@ class ClockSampler:
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
-        # samples under load = upper half of the observed clocks' activity window
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_rate(cfg, nu, w, phi, q_los, u_los, target_s=12.0):
+def oracle_rate(cfg, nu, w, phi, q_los, u_los, target_s=15.0):
     """FP64 oracle as it stands, all host cores, on a bounded sample of the workload's pixels."""
     import oracle
     op = oracle.make_plan(nu, w, phi)
-    n0 = min(64, q_los.shape[0])
+    n0 = min(2048, q_los.shape[0])
     t0 = time.perf_counter()
     oracle.synth_table(op, q_los[:n0], u_los[:n0])
     dt = max(time.perf_counter() - t0, 1e-4)
@@ -94,7 +97,7 @@ def oracle_rate(cfg, nu, w, phi, q_los, u_los, target_s=12.0):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
     ap.add_argument("--scheme", default="tf32x3", choices=["tf32x3", "fp32_table", "fp32_sincos"])
@@ -155,9 +158,13 @@ def main():
     scheme = {"tf32x3": b.SCHEME_TF32X3, "fp32_table": b.SCHEME_FP32_TABLE, "fp32_sincos": b.SCHEME_FP32_SINCOS}[a.scheme]
     layout = (b.IN_FREQ_MAJOR if cfg.layout_in == "freq" else 0) | (b.OUT_PHI_MAJOR if cfg.layout_out == "phi" else 0)
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()          # started early: nvidia-smi needs ~1 s before its first sample
     # each rank owns an independent cube (weak scaling): same grids, different pixel seeds via the rank offset
     import dataclasses
-    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    from paper_1810_06250_b200 import sharding
+    rcfg = dataclasses.replace(cfg, seed=sharding.rank_seed(cfg.seed, rank))
     Q, U = ri.generate_cube(rcfg, "cuda")
     out_shape = (cfg.n_phi, cfg.n_pix) if cfg.layout_out == "phi" else (cfg.n_pix, cfg.n_phi)
     FQ = torch.empty(out_shape, device="cuda")
@@ -184,28 +191,22 @@ def main():
     for _ in range(max(a.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     b.rmsynth_launch_count(True)
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps + 1)]
     barrier()
+    t_begin = time.time()
     evs[0].record()
     for i in range(a.steps):
         step()
         evs[i + 1].record()
     barrier()
+    t_end = time.time()
     launches = b.rmsynth_launch_count()
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = evs[0].elapsed_time(evs[-1])
+    clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
+    total_ms = sharding.max_over_ranks(evs[0].elapsed_time(evs[-1]), "cuda")
     per_step = [evs[i].elapsed_time(evs[i + 1]) for i in range(a.steps)]
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
     ms_step = total_ms / a.steps
-    value = world * cfg.cmac / (ms_step * 1e-3) / 1e9
+    value = sharding.whole_job_rate(cfg.cmac, ms_step * 1e-3, world) / 1e9
 
     # ---- end-to-end through the host-buffer API (pinned memory, H2D + D2H inside the timed region)
     e2e = None
@@ -220,12 +221,7 @@ def main():
         for _ in range(k_e2e):
             plan.execute_host(hQ, hU, cfg.n_pix, layout, hFQ, hFU)
         torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / k_e2e
-        if world > 1:
-            import torch.distributed as dist
-            t = torch.tensor([dt], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = sharding.max_over_ranks((time.perf_counter() - t0) / k_e2e, "cuda")
         ok = bool(torch.equal(hFQ.cuda(), FQ)) if scheme != b.SCHEME_FP32_SINCOS else True
         e2e = {"value": world * cfg.cmac / dt / 1e9, "unit": "GCMAC/s", "h2d_bytes_per_step": 2 * hQ.numel() * 4,
                "d2h_bytes_per_step": 2 * hFQ.numel() * 4, "ms_per_step": dt * 1e3, "steps": k_e2e,
@@ -258,7 +254,7 @@ def main():
         import oracle
         oracle.build()
         rng = np.random.default_rng(0)
-        pix = np.sort(rng.choice(cfg.n_pix, size=min(cfg.n_pix, 65536), replace=False))
+        pix = np.sort(rng.choice(cfg.n_pix, size=min(cfg.n_pix, 262144), replace=False))
         q_los, u_los = ri.gather_los(Q, U, cfg.layout_in, pix)
         rate, threads, n, dt = oracle_rate(cfg, nu, w, phi, q_los, u_los)
         cpu = {"value": rate, "unit": "GCMAC/s", "cores": threads, "kind": "oracle",

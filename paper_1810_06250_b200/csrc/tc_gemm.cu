@@ -178,11 +178,12 @@ struct TcParams {
     float* FU;
 };
 
-template <int KS, int IN_MN>
+template <int KS, int IN_MN, int OUT_LOS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU, const TcParams prm) {
     using Cfg = TcCfg<KS>;
-    constexpr int S = Cfg::kStages;
+    // LOS-major output gives one ring stage to the per-warp transpose buffers of the epilogue
+    constexpr int S = OUT_LOS ? Cfg::kStages - 1 : Cfg::kStages;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
@@ -194,6 +195,7 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
     uint64_t* acc_full = bars + 3 * S;   // [2] chunk accumulated       (count 1, tcgen05.commit)
     uint64_t* acc_empty = acc_full + 2;  // [2] chunk drained           (count 256)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+    float* stage_t = reinterpret_cast<float*>(smem_gen + (size_t)S * Cfg::kStageBytes + 1024);   // 8 x [32][33] floats
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = prm.n, N2 = 2 * prm.n;
@@ -367,15 +369,17 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                     mbar_arrive(&acc_empty[ab]);
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
-                if (p < prm.n_pix) {
-                    // my columns cbase..cbase+127 of [FQ(0..n) | FU(n..2n)]; nv depths of this tile are real.
-                    // All bounds are warp-uniform; addresses are base + i*stride with compile-time i.
-                    const int nv = min(n, prm.n_phi - j * n);
-                    const int q_end = nv - cbase, u_beg = n - cbase, u_end = n + nv - cbase;
-                    const long long sb = prm.out_phi_major ? 4LL * prm.n_pix : 4LL;   // byte stride between depths
-                    const long long kq = (long long)j * n + cbase, ku = kq - n;
-                    unsigned long long aq = (unsigned long long)(prm.FQ + (prm.out_phi_major ? kq * prm.n_pix + p : p * prm.n_phi + kq));
-                    unsigned long long au = (unsigned long long)(prm.FU + (prm.out_phi_major ? ku * prm.n_pix + p : p * prm.n_phi + ku));
+                // my columns cbase..cbase+127 of [FQ(0..n) | FU(n..2n)]; nv depths of this tile are real.
+                const int nv = min(n, prm.n_phi - j * n);
+                const int q_end = nv - cbase, u_beg = n - cbase, u_end = n + nv - cbase;
+                const long long kq = (long long)j * n + cbase, ku = kq - n;
+                if (!OUT_LOS) {
+                  if (p < prm.n_pix) {
+                    // phi-major: a warp writes 128 contiguous bytes per depth.  All bounds are warp-uniform;
+                    // addresses are base + i*stride with compile-time i, stores predicated (no branches).
+                    const long long sb = 4LL * prm.n_pix;   // byte stride between depths
+                    unsigned long long aq = (unsigned long long)(prm.FQ + kq * prm.n_pix + p);
+                    unsigned long long au = (unsigned long long)(prm.FU + ku * prm.n_pix + p);
                     asm volatile("" : "+l"(aq), "+l"(au));   // keep the bases in registers (no rematerialisation)
 #pragma unroll
                     for (int g = 0; g < 4; ++g) {
@@ -388,6 +392,29 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
 #pragma unroll
                             for (int i = g * 32; i < g * 32 + 32; ++i)
                                 st_global_pred(au + i * sb, acc[i], (unsigned)(i - u_beg) < (unsigned)nv);
+                        }
+                    }
+                  }
+                } else {
+                    // LOS-major: transpose 32x32 blocks through a private smem buffer so that each store
+                    // instruction writes 32 consecutive depths of ONE pixel row (128 contiguous bytes).
+                    float* sT = stage_t + (warp - 8) * (32 * 33);
+                    const long long P0 = (long long)t * TC_M + q * 32;              // first pixel of this warp
+                    const int rows = (int)min(32LL, prm.n_pix - P0);                // ragged last tile (may be <= 0)
+                    const long long rb = 4LL * prm.n_phi;                           // byte stride between pixel rows
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        const int i = g * 32 + lane;                                 // the column this lane stores
+                        const bool is_q = i < q_end, is_u = (unsigned)(i - u_beg) < (unsigned)nv;
+                        if (g * 32 < q_end || (g * 32 + 32 > u_beg && g * 32 < u_end)) {   // warp-uniform
+#pragma unroll
+                            for (int c = 0; c < 32; ++c) sT[lane * 33 + c] = acc[g * 32 + c];
+                            __syncwarp();
+                            unsigned long long a = (unsigned long long)((is_u ? prm.FU + ku : prm.FQ + kq) + P0 * prm.n_phi + i);
+#pragma unroll 8
+                            for (int r = 0; r < 32; ++r)
+                                st_global_pred(a + r * rb, sT[r * 33 + lane], (is_q || is_u) && r < rows);
+                            __syncwarp();
                         }
                     }
                 }
@@ -432,8 +459,10 @@ rmsynth_status tc_plan_init(rmsynth_plan* p) {
     dim3 grid((g.n_tile + 63) / 64, n_stages, g.n_phi_tiles);
     tc_build_b_kernel<TC_KS><<<grid, 64>>>(p->d_delta, p->d_kw, p->d_phi, p->n_chan, p->n_phi, g.n_tile, n_stages, p->d_tcB);
     RMS_LAUNCH_CHECK("tc_build_b_kernel");
-    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
-    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+    RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
     return RMSYNTH_OK;
 }
 
@@ -543,10 +572,10 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     if (want_prof) {
         RMS_CUDA(cudaMalloc(&prm.prof, sizeof(long long) * 4 * grid));
     }
-    if (in_freq)
-        tc_rmsynth_kernel<TC_KS, 1><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
-    else
-        tc_rmsynth_kernel<TC_KS, 0><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
+    if (in_freq && out_phi) tc_rmsynth_kernel<TC_KS, 1, 0><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
+    else if (in_freq) tc_rmsynth_kernel<TC_KS, 1, 1><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
+    else if (out_phi) tc_rmsynth_kernel<TC_KS, 0, 0><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
+    else tc_rmsynth_kernel<TC_KS, 0, 1><<<grid, TC_THREADS, Cfg::kSmemBytes, st>>>(mq, mu_, prm);
     RMS_LAUNCH_CHECK("tc_rmsynth_kernel");
     if (want_prof) {   // debug only: synchronises
         std::vector<long long> h(4 * grid);

@@ -251,3 +251,47 @@ def test_nonfinite_samples_stay_in_their_pixel(b):
         bad = ~(torch.isfinite(fq).all(1) & torch.isfinite(fu).all(1))
         assert sorted(torch.nonzero(bad).flatten().tolist()) == [17, 150], scheme
         plan.destroy()
+
+
+# ------------------------------------------------------------------ full BASELINE sizes, bench launch configuration
+@pytest.mark.parametrize("cfg_id", [2, 4, 3, 5])
+def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id):
+    """The cube bench.py times (same layouts, same scheme, one rmsynth_execute_peaks call over the whole
+    cube), checked on lines of sight the oracle can compute one by one: every pixel of the first and last
+    tile, tile-boundary neighbours and a random sample; plus properties that hold at any size."""
+    cfg = ri.CONFIGS[cfg_id]
+    nu, w, phi = ri.grids(cfg)
+    Q, U = ri.generate_cube(cfg, "cuda")
+    layout = (b.IN_FREQ_MAJOR if cfg.layout_in == "freq" else 0) | (b.OUT_PHI_MAJOR if cfg.layout_out == "phi" else 0)
+    shape = (cfg.n_phi, cfg.n_pix) if cfg.layout_out == "phi" else (cfg.n_pix, cfg.n_phi)
+    FQ = torch.full(shape, float("nan"), device="cuda")
+    FU = torch.full(shape, float("nan"), device="cuda")
+    maps = {k: torch.full((cfg.n_pix,), float("nan"), device="cuda") for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero")}
+    maps["peak_index"] = torch.full((cfg.n_pix,), -1, dtype=torch.int32, device="cuda")
+    plan = b.Plan(nu, w, phi)                                   # default scheme = the product path
+    plan.execute_peaks(Q, U, cfg.n_pix, layout, FQ, FU, **maps)
+    torch.cuda.synchronize()
+    # properties at full size: every output written and finite, |F| <= T_p (triangle inequality), index in range
+    assert bool(torch.isfinite(FQ).all()) and bool(torch.isfinite(FU).all())
+    assert int(maps["peak_index"].min()) >= 0 and int(maps["peak_index"].max()) < cfg.n_phi
+    kw = torch.as_tensor(plan.K * w, dtype=torch.float32, device="cuda")
+    amp_in = torch.sqrt(Q * Q + U * U)
+    T_all = (amp_in * (kw[:, None] if cfg.layout_in == "freq" else kw[None, :])).sum(0 if cfg.layout_in == "freq" else 1)
+    Fmax = torch.sqrt(FQ * FQ + FU * FU).amax(0 if cfg.layout_out == "phi" else 1)
+    assert bool((Fmax <= T_all * (1 + 1e-4) + 1e-30).all())
+    del amp_in
+    # sampled lines of sight against the oracle
+    rng = np.random.default_rng(cfg_id)
+    n = cfg.n_pix
+    pix = np.unique(np.concatenate([np.arange(0, 128), np.arange(n - 128, n), np.arange(127, n, max(n // 64, 128))[:64],
+                                    np.arange(128, n, max(n // 64, 128))[:64], rng.choice(n, 256, replace=False)]))
+    q, u = ri.gather_los(Q, U, cfg.layout_in, pix)
+    op, oFQ, oFU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    idx = torch.as_tensor(pix, device="cuda")
+    gq = (FQ.index_select(1, idx).T if cfg.layout_out == "phi" else FQ.index_select(0, idx)).cpu().numpy()
+    gu = (FU.index_select(1, idx).T if cfg.layout_out == "phi" else FU.index_select(0, idx)).cpu().numpy()
+    worst = check_cubes(gq, gu, oFQ, oFU, T, f"full config {cfg_id}")
+    got = {("kstar" if k == "peak_index" else k): v.index_select(0, idx).cpu().numpy() for k, v in maps.items()}
+    check_peaks(oracle_mod, op, oFQ, oFU, T, got, cfg.dphi, f"full config {cfg_id}")
+    print(f"full config {cfg_id}: {pix.size} sampled lines of sight, max err/T_p = {worst:.2e}")
+    plan.destroy()
