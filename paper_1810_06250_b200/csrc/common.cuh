@@ -37,6 +37,7 @@ struct TcGeom {
     int n_phi_tiles = 0; // ceil(n_phi / n)
     int k_pad = 0;       // n_chan rounded up to the K block
     int kb = 0;          // channels per K block
+    int ctas = 1;        // 1: tc_gemm.cu (cta_group::1), 2: tc_gemm2.cu (CTA pairs, cta_group::2)
 };
 
 }  // namespace rms
@@ -61,7 +62,8 @@ struct rmsynth_plan {
     float2* d_phi2 = nullptr;             // phi as hi+lo floats              [n_phi]
     // tensor path (tc_gemm.cu)
     rms::TcGeom tc;
-    float* d_tcB = nullptr;               // pre-split, tiled B operand
+    float* d_tcB = nullptr;               // pre-split, tiled B operand (cta_group::1 layout)
+    float* d_tcB2 = nullptr;              // same for CTA pairs
     void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
@@ -90,5 +92,10 @@ void tc_plan_free(rmsynth_plan* p);
 rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
                           float* FQ, float* FU, float* amp, float* phi, float* pa0, float* paz, int* idx,
                           cudaStream_t st);
+
+// tc_gemm2.cu
+rmsynth_status tc2_plan_init(rmsynth_plan* p);
+rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
+                          bool out_phi, long long n_pix, float* FQ, float* FU, cudaStream_t st);
 
 }  // namespace rms

@@ -24,6 +24,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include "common.cuh"
+#include "tc_common.cuh"
 
 namespace rms {
 
@@ -45,82 +46,6 @@ template <int KS> struct TcCfg {
     static constexpr int kStagesPerChunk = TC_CHUNK / KS;
     static constexpr int kKSteps = KS / 8;                        // MMAs (K=8) per operand pair per stage
 };
-
-// ------------------------------------------------------------------------------------------------
-// PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc),
-        "r"(acc) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
-        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr));
-}
-__device__ __forceinline__ void st_global_pred(unsigned long long addr, float v, bool pred) {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %2, 0;\n@p st.global.f32 [%0], %1;\n}" ::"l"(addr), "f"(v), "r"((int)pred) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-// UMMA shared-memory matrix descriptor (version 1 = sm_100).  Offsets in bytes.
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo, uint32_t layout_type) {
-    uint64_t d = 0;
-    d |= (uint64_t)((saddr >> 4) & 0x3FFF);
-    d |= (uint64_t)((lbo >> 4) & 0x3FFF) << 16;
-    d |= (uint64_t)((sbo >> 4) & 0x3FFF) << 32;
-    d |= (uint64_t)1 << 46;
-    d |= (uint64_t)layout_type << 61;
-    return d;
-}
-
-__device__ __forceinline__ float rn_tf32(float x) {   // round-to-nearest(-even) to 10 explicit mantissa bits
-    uint32_t u = __float_as_uint(x);
-    if ((u & 0x7F800000u) == 0x7F800000u) return x;
-    u += 0xFFFu + ((u >> 13) & 1u);
-    return __uint_as_float(u & 0xFFFFE000u);
-}
 
 // ------------------------------------------------------------------------------------------------
 // Plan time: the pre-split, pre-swizzled B operand.  One blob per (depth tile j, K stage s):
@@ -190,10 +115,10 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
     // stage layout: [Qraw][Uraw][Qlo][Ulo][B hi part][B lo part]
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_gen + (size_t)S * Cfg::kStageBytes);
     uint64_t* full = bars;               // TMA bytes landed            (count 1 + tx)
-    uint64_t* ready = bars + S;          // A_lo written                (count 128)
+    uint64_t* ready = bars + S;          // A_lo written                (count 4: one per transform warp)
     uint64_t* empty = bars + 2 * S;      // MMAs that read the stage done (count 1, tcgen05.commit)
     uint64_t* acc_full = bars + 3 * S;   // [2] chunk accumulated       (count 1, tcgen05.commit)
-    uint64_t* acc_empty = acc_full + 2;  // [2] chunk drained           (count 256)
+    uint64_t* acc_empty = acc_full + 2;  // [2] chunk drained           (count 8: one per epilogue warp)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
     float* stage_t = reinterpret_cast<float*>(smem_gen + (size_t)S * Cfg::kStageBytes + 1024);   // 8 x [32][33] floats
 
@@ -204,8 +129,8 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
     const int n_chunks = (prm.n_stages + Cfg::kStagesPerChunk - 1) / Cfg::kStagesPerChunk;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&ready[s], 128); mbar_init(&empty[s], 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], 256); }
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&ready[s], 4); mbar_init(&empty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], 8); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -332,7 +257,8 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                 *reinterpret_cast<float4*>(sg + 2 * Cfg::kAPart + o) = l;
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_arrive(&ready[st]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ready[st]);
             if (++st == S) { st = 0; ph ^= 1; }
         }
     } else {
@@ -366,7 +292,8 @@ tc_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                         }
                     }
                     tc_fence_before();
-                    mbar_arrive(&acc_empty[ab]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&acc_empty[ab]);
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
                 // my columns cbase..cbase+127 of [FQ(0..n) | FU(n..2n)]; nv depths of this tile are real.
@@ -463,12 +390,16 @@ rmsynth_status tc_plan_init(rmsynth_plan* p) {
     RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
     RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
     RMS_CUDA(cudaFuncSetAttribute(tc_rmsynth_kernel<TC_KS, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+    const char* mode = getenv("RMSYNTH_TC_CTAS");      // "1" = single-CTA kernel, default = CTA pairs
+    g.ctas = (mode && mode[0] == '1') ? 1 : 2;
+    if (g.ctas == 2) return tc2_plan_init(p);
     return RMSYNTH_OK;
 }
 
 void tc_plan_free(rmsynth_plan* p) {
     if (p->d_tcB) cudaFree(p->d_tcB);
-    p->d_tcB = nullptr;
+    if (p->d_tcB2) cudaFree(p->d_tcB2);
+    p->d_tcB = p->d_tcB2 = nullptr;
 }
 
 // Copy a cube into a buffer whose row pitch is a multiple of 4 floats (TMA needs 16-byte strides).
@@ -551,6 +482,11 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
         if ((s = make_map(&mq, Q, p->n_chan, n_pix, pitch, TC_KS, TC_M, sw)) ||
             (s = make_map(&mu_, U, p->n_chan, n_pix, pitch, TC_KS, TC_M, sw)))
             return s;
+    }
+    if (p->tc.ctas == 2) {
+        if ((s = tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, st))) return s;
+        if (!want_maps) return RMSYNTH_OK;
+        return peaks_from_cubes(p, FQ, FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, amp, phi, pa0, paz, idx, st);
     }
     TcParams prm;
     prm.n_pix = n_pix;
