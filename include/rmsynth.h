@@ -113,6 +113,23 @@ rmsynth_status rmsynth_execute_peaks(const rmsynth_plan *plan, const float *Q, c
                                      float *peak_amp, float *peak_phi, float *pa_lambda0,
                                      float *pa_zero, int *peak_index, void *stream);
 
+/* Every output of the path in one call (NEXT-1 of the scope table: the paper's third cube).
+ * Any subset may be requested; at least one pointer must be non-NULL.
+ *   FQ, FU     DEVICE cubes, both or neither
+ *   F_abs      DEVICE cube |F| = sqrt(FQ^2 + FU^2) (Eq. 17; cuFFS writes it as a third
+ *              cube), same layout as FQ/FU; formed in FP32 from the FP32 FQ, FU
+ *   peak_*     as in rmsynth_execute_peaks
+ * With FQ = FU = F_abs = NULL no cube is written at all ("maps only": half of the HBM traffic). */
+typedef struct {
+    int struct_size;                 /* sizeof(rmsynth_outputs) */
+    float *FQ, *FU, *F_abs;
+    float *peak_amp, *peak_phi, *pa_lambda0, *pa_zero;
+    int *peak_index;
+} rmsynth_outputs;
+rmsynth_status rmsynth_execute_ex(const rmsynth_plan *plan, const float *Q, const float *U,
+                                  long long n_pix, int layout, const rmsynth_outputs *out,
+                                  void *stream);
+
 /* Same as rmsynth_execute_peaks with every cube/map pointer in HOST memory (pinned memory
  * gives full PCIe rate): the library streams pixel chunks host->device->host through its own
  * device buffers, overlapping copies with compute, and returns when the outputs are complete.

@@ -22,13 +22,19 @@ IN_LOS_MAJOR, IN_FREQ_MAJOR, OUT_LOS_MAJOR, OUT_PHI_MAJOR = 0, 1, 0, 2
 SCHEME_AUTO, SCHEME_TF32X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS = 0, 1, 3, 4
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
-           "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_host", "rmsynth_rmsf",
+           "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_rmsf",
            "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
 
 
 class Options(C.Structure):
     _fields_ = [("struct_size", C.c_int), ("scheme", C.c_int), ("lambda0_mode", C.c_int),
                 ("device", C.c_int), ("lambda0_sq", C.c_double)]
+
+
+class Outputs(C.Structure):
+    _fields_ = [("struct_size", C.c_int), ("FQ", C.c_void_p), ("FU", C.c_void_p), ("F_abs", C.c_void_p),
+                ("peak_amp", C.c_void_p), ("peak_phi", C.c_void_p), ("pa_lambda0", C.c_void_p),
+                ("pa_zero", C.c_void_p), ("peak_index", C.c_void_p)]
 
 
 _dp, _fp, _ip, _vp = C.POINTER(C.c_double), C.c_void_p, C.c_void_p, C.c_void_p
@@ -38,6 +44,7 @@ _lib.rmsynth_plan_info.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int), C.POINTER(
 _lib.rmsynth_plan_phase_matrix.argtypes = [_vp, _vp, _vp]
 _lib.rmsynth_execute.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _vp]
 _lib.rmsynth_execute_peaks.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
+_lib.rmsynth_execute_ex.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, C.POINTER(Outputs), _vp]
 _lib.rmsynth_execute_host.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip]
 _lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
 _lib.rmsynth_launch_count.argtypes = [C.c_int]
@@ -128,6 +135,13 @@ class Plan:
         _check(_lib.rmsynth_execute_peaks(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
                                           _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
                                           _ptr(peak_index), stream))
+
+    def execute_ex(self, Q, U, n_pix, layout, FQ=None, FU=None, F_abs=None, peak_amp=None, peak_phi=None,
+                   pa_lambda0=None, pa_zero=None, peak_index=None, stream=None):
+        """Any subset of the outputs (cubes FQ/FU, |F| cube, maps) in one call; all DEVICE tensors."""
+        out = Outputs(C.sizeof(Outputs), _ptr(FQ), _ptr(FU), _ptr(F_abs), _ptr(peak_amp), _ptr(peak_phi),
+                      _ptr(pa_lambda0), _ptr(pa_zero), _ptr(peak_index))
+        _check(_lib.rmsynth_execute_ex(self._h, _ptr(Q), _ptr(U), n_pix, layout, C.byref(out), stream))
 
     def execute_host(self, Q, U, n_pix, layout, FQ=None, FU=None, peak_amp=None, peak_phi=None,
                      pa_lambda0=None, pa_zero=None, peak_index=None):

@@ -37,7 +37,7 @@ struct TcGeom {
     int n_phi_tiles = 0; // ceil(n_phi / n)
     int k_pad = 0;       // n_chan rounded up to the K block
     int kb = 0;          // channels per K block
-    int ctas = 1;        // 1: tc_gemm.cu (cta_group::1), 2: tc_gemm2.cu (CTA pairs, cta_group::2)
+    int ctas = 2;        // CTA pairs (tcgen05 cta_group::2)
 };
 
 }  // namespace rms
@@ -62,20 +62,25 @@ struct rmsynth_plan {
     float2* d_phi2 = nullptr;             // phi as hi+lo floats              [n_phi]
     // tensor path (tc_gemm.cu)
     rms::TcGeom tc;
-    float* d_tcB = nullptr;               // pre-split, tiled B operand (cta_group::1 layout)
-    float* d_tcB2 = nullptr;              // same for CTA pairs
+    float* d_tcB2 = nullptr;              // pre-split, pre-swizzled B operand blobs (tc_gemm2.cu)
     void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
-    static constexpr int kScratch = 14;   // 0-7 host-stream slots (Q,U,FQ,FU x2); 8,9 their maps; 10,11 maps-only cubes; 12,13 TMA repack
+    static constexpr int kScratch = 10;   // 0-7 host-stream slots (Q,U,FQ,FU x2); 8,9 their maps
     mutable float* scratch[kScratch] = {};
     mutable size_t scratch_bytes[kScratch] = {};
+    // per-call workspace keyed by (stream, tag) so that concurrent calls on different streams never share it
+    struct StreamScratch { cudaStream_t st; int tag; float* ptr; size_t bytes; };
+    mutable std::mutex pool_mu;
+    mutable std::vector<StreamScratch> pool;
     mutable cudaStream_t hs[2] = {nullptr, nullptr};
 };
 
 namespace rms {
 
 rmsynth_status ensure_scratch(const rmsynth_plan* p, int slot, size_t bytes, float** out);
+enum { SCR_PEAK_REC = 0, SCR_CUBE_Q = 1, SCR_CUBE_U = 2, SCR_REPACK_Q = 3, SCR_REPACK_U = 4 };
+rmsynth_status stream_scratch(const rmsynth_plan* p, cudaStream_t st, int tag, size_t bytes, float** out);
 
 // fp32_kernels.cu
 rmsynth_status fp32_table_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
@@ -83,6 +88,9 @@ rmsynth_status fp32_table_execute(const rmsynth_plan* p, const float* Q, const f
 rmsynth_status fp32_sincos_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
                                    int layout, float* FQ, float* FU, cudaStream_t st);
 // peaks.cu
+rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,
+                             float* pa0, float* paz, int* idx, cudaStream_t st);
+rmsynth_status abs_from_cubes(const float* FQ, const float* FU, long long n, float* FA, cudaStream_t st);
 rmsynth_status peaks_from_cubes(const rmsynth_plan* p, const float* FQ, const float* FU, long long n_pix,
                                 int out_layout, float* amp, float* phi, float* pa0, float* paz, int* idx,
                                 cudaStream_t st);
@@ -90,12 +98,12 @@ rmsynth_status peaks_from_cubes(const rmsynth_plan* p, const float* FQ, const fl
 rmsynth_status tc_plan_init(rmsynth_plan* p);
 void tc_plan_free(rmsynth_plan* p);
 rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
-                          float* FQ, float* FU, float* amp, float* phi, float* pa0, float* paz, int* idx,
+                          float* FQ, float* FU, float* FA, float* amp, float* phi, float* pa0, float* paz, int* idx,
                           cudaStream_t st);
 
 // tc_gemm2.cu
 rmsynth_status tc2_plan_init(rmsynth_plan* p);
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, cudaStream_t st);
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st);
 
 }  // namespace rms

@@ -1,42 +1,50 @@
-// rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_host: argument checks, scheme
-// dispatch (rows a4-a9) and the host-streaming loop (the paper's "each datum crosses the bus
+// rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_ex / rmsynth_execute_host: argument checks,
+// scheme dispatch (rows a4-a9) and the host-streaming loop (the paper's "each datum crosses the bus
 // once" rule, with pixel chunks instead of LOS batches sized from GPU memory P:L210).
+#include <cstring>
 #include "common.cuh"
 
 namespace rms {
 
+struct Outs {
+    float *FQ = nullptr, *FU = nullptr, *FA = nullptr;
+    float *amp = nullptr, *phi = nullptr, *pa0 = nullptr, *paz = nullptr;
+    int* idx = nullptr;
+    bool maps() const { return amp || phi || pa0 || paz || idx; }
+    bool any() const { return FQ || FA || maps(); }
+};
+
 static rmsynth_status check_args(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
-                                 int layout, bool need_cubes, const float* FQ, const float* FU) {
+                                 int layout, bool need_cubes, const Outs& o) {
     if (!p) return fail(RMSYNTH_EINVAL, "plan is NULL");
     if (n_pix < 0) return fail(RMSYNTH_EINVAL, "n_pix < 0");
     if (layout & ~3) return fail(RMSYNTH_EINVAL, "unknown layout flags");
     if (n_pix == 0) return RMSYNTH_OK;
     if (!Q || !U) return fail(RMSYNTH_EINVAL, "Q/U is NULL");
-    if ((FQ == nullptr) != (FU == nullptr)) return fail(RMSYNTH_EINVAL, "FQ and FU must both be given or both NULL");
-    if (need_cubes && !FQ) return fail(RMSYNTH_EINVAL, "FQ/FU is NULL");
+    if ((o.FQ == nullptr) != (o.FU == nullptr)) return fail(RMSYNTH_EINVAL, "FQ and FU must both be given or both NULL");
+    if (need_cubes && !o.FQ) return fail(RMSYNTH_EINVAL, "FQ/FU is NULL");
+    if (!o.any()) return fail(RMSYNTH_EINVAL, "no output requested");
     if (n_pix > (1LL << 40)) return fail(RMSYNTH_EINVAL, "n_pix too large");
     return RMSYNTH_OK;
 }
 
-// Device-resident contraction + optional maps on one stream; never synchronises.
+// Device-resident contraction + optional |F| cube and maps on one stream; never synchronises.
 static rmsynth_status run_device(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
-                                 float* FQ, float* FU, float* amp, float* phi, float* pa0, float* paz, int* idx,
-                                 cudaStream_t st) {
-    const bool want_maps = amp || phi || pa0 || paz || idx;
+                                 Outs o, cudaStream_t st) {
     if (p->scheme == RMSYNTH_SCHEME_TF32X3)
-        return tc_execute(p, Q, U, n_pix, layout, FQ, FU, amp, phi, pa0, paz, idx, st);
-    // FP32 CUDA-core comparison paths: cubes first, then the stand-alone peak kernel.
-    if (!FQ) {
-        std::lock_guard<std::mutex> g(p->mu);
+        return tc_execute(p, Q, U, n_pix, layout, o.FQ, o.FU, o.FA, o.amp, o.phi, o.pa0, o.paz, o.idx, st);
+    // FP32 CUDA-core comparison paths: cubes first, then the stand-alone |F| and peak kernels.
+    rmsynth_status s;
+    if (!o.FQ) {
         size_t bytes = sizeof(float) * (size_t)n_pix * p->n_phi;
-        rmsynth_status s;
-        if ((s = ensure_scratch(p, 10, bytes, &FQ)) || (s = ensure_scratch(p, 11, bytes, &FU))) return s;
+        if ((s = stream_scratch(p, st, SCR_CUBE_Q, bytes, &o.FQ)) || (s = stream_scratch(p, st, SCR_CUBE_U, bytes, &o.FU)))
+            return s;
     }
-    rmsynth_status s = p->scheme == RMSYNTH_SCHEME_FP32_TABLE
-                           ? fp32_table_execute(p, Q, U, n_pix, layout, FQ, FU, st)
-                           : fp32_sincos_execute(p, Q, U, n_pix, layout, FQ, FU, st);
-    if (s != RMSYNTH_OK || !want_maps) return s;
-    return peaks_from_cubes(p, FQ, FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, amp, phi, pa0, paz, idx, st);
+    s = p->scheme == RMSYNTH_SCHEME_FP32_TABLE ? fp32_table_execute(p, Q, U, n_pix, layout, o.FQ, o.FU, st)
+                                               : fp32_sincos_execute(p, Q, U, n_pix, layout, o.FQ, o.FU, st);
+    if (s == RMSYNTH_OK && o.FA) s = abs_from_cubes(o.FQ, o.FU, n_pix * p->n_phi, o.FA, st);
+    if (s != RMSYNTH_OK || !o.maps()) return s;
+    return peaks_from_cubes(p, o.FQ, o.FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, o.amp, o.phi, o.pa0, o.paz, o.idx, st);
 }
 
 }  // namespace rms
@@ -47,31 +55,43 @@ extern "C" {
 
 rmsynth_status rmsynth_execute(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
                                int layout, float* FQ, float* FU, void* stream) {
-    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, true, FQ, FU);
+    Outs o;
+    o.FQ = FQ;
+    o.FU = FU;
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, true, o);
     if (s != RMSYNTH_OK || n_pix == 0) return s;
-    return run_device(plan, Q, U, n_pix, layout, FQ, FU, nullptr, nullptr, nullptr, nullptr, nullptr,
-                      (cudaStream_t)stream);
+    return run_device(plan, Q, U, n_pix, layout, o, (cudaStream_t)stream);
 }
 
 rmsynth_status rmsynth_execute_peaks(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
                                      int layout, float* FQ, float* FU, float* peak_amp, float* peak_phi,
                                      float* pa_lambda0, float* pa_zero, int* peak_index, void* stream) {
-    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, FQ, FU);
+    Outs o;
+    o.FQ = FQ; o.FU = FU; o.amp = peak_amp; o.phi = peak_phi; o.pa0 = pa_lambda0; o.paz = pa_zero; o.idx = peak_index;
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, o);
     if (s != RMSYNTH_OK || n_pix == 0) return s;
-    if (!FQ && !(peak_amp || peak_phi || pa_lambda0 || pa_zero || peak_index))
-        return fail(RMSYNTH_EINVAL, "no output requested");
-    return run_device(plan, Q, U, n_pix, layout, FQ, FU, peak_amp, peak_phi, pa_lambda0, pa_zero, peak_index,
-                      (cudaStream_t)stream);
+    return run_device(plan, Q, U, n_pix, layout, o, (cudaStream_t)stream);
+}
+
+rmsynth_status rmsynth_execute_ex(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
+                                  int layout, const rmsynth_outputs* out, void* stream) {
+    if (!out || out->struct_size != (int)sizeof(rmsynth_outputs)) return fail(RMSYNTH_EINVAL, "outputs.struct_size");
+    Outs o;
+    o.FQ = out->FQ; o.FU = out->FU; o.FA = out->F_abs; o.amp = out->peak_amp; o.phi = out->peak_phi;
+    o.pa0 = out->pa_lambda0; o.paz = out->pa_zero; o.idx = out->peak_index;
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, o);
+    if (s != RMSYNTH_OK || n_pix == 0) return s;
+    return run_device(plan, Q, U, n_pix, layout, o, (cudaStream_t)stream);
 }
 
 rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, const float* U, long long n_pix,
                                     int layout, float* FQ, float* FU, float* peak_amp, float* peak_phi,
                                     float* pa_lambda0, float* pa_zero, int* peak_index) {
-    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, FQ, FU);
+    Outs ho;
+    ho.FQ = FQ; ho.FU = FU; ho.amp = peak_amp; ho.phi = peak_phi; ho.pa0 = pa_lambda0; ho.paz = pa_zero; ho.idx = peak_index;
+    rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, ho);
     if (s != RMSYNTH_OK || n_pix == 0) return s;
     const rmsynth_plan* p = plan;
-    const bool want_maps = peak_amp || peak_phi || pa_lambda0 || pa_zero || peak_index;
-    if (!FQ && !want_maps) return fail(RMSYNTH_EINVAL, "no output requested");
     RMS_CUDA(cudaSetDevice(p->device));
     std::lock_guard<std::mutex> g(p->mu);
     const int nc = p->n_chan, np = p->n_phi;
@@ -104,9 +124,14 @@ rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, co
             RMS_CUDA(cudaMemcpyAsync(dU[b], U + p0 * nc, sizeof(float) * n * nc, cudaMemcpyHostToDevice, st));
         }
         float* m = dM[b];
-        s = run_device(p, dQ[b], dU[b], n, layout, dFQ[b], dFU[b], peak_amp ? m : nullptr,
-                       peak_phi ? m + chunk : nullptr, pa_lambda0 ? m + 2 * chunk : nullptr,
-                       pa_zero ? m + 3 * chunk : nullptr, peak_index ? (int*)(m + 4 * chunk) : nullptr, st);
+        Outs o;
+        if (FQ) { o.FQ = dFQ[b]; o.FU = dFU[b]; }
+        o.amp = peak_amp ? m : nullptr;
+        o.phi = peak_phi ? m + chunk : nullptr;
+        o.pa0 = pa_lambda0 ? m + 2 * chunk : nullptr;
+        o.paz = pa_zero ? m + 3 * chunk : nullptr;
+        o.idx = peak_index ? (int*)(m + 4 * chunk) : nullptr;
+        s = run_device(p, dQ[b], dU[b], n, layout, o, st);
         if (s != RMSYNTH_OK) return s;
         if (FQ) {
             if (out_phi) {

@@ -7,6 +7,7 @@
 // same refine_and_store() so both paths take the integer decision in the same precision.
 #include "common.cuh"
 #include "peak_refine.cuh"
+#include "tc_epilogue.cuh"
 
 namespace rms {
 
@@ -57,6 +58,68 @@ __global__ void __launch_bounds__(256) peaks_los_major_kernel(
     if (kb > 0) { float q = fq[kb - 1], u = fu[kb - 1]; s.best_ym2 = fmaf(q, q, u * u); }
     if (kb < n_phi - 1) { float q = fq[kb + 1], u = fu[kb + 1]; s.best_yp2 = fmaf(q, q, u * u); }
     refine_and_store(s, n_phi, phif, lambda0_sq, p, amp, phi, pa0, paz, idx);
+}
+
+// Row a7, fused form: merge the per-segment records the tensor kernel's epilogue wrote (tc_epilogue.cuh) --
+// segments of a pixel are visited in ascending depth order with a strict >, so the decision sequence is the
+// one a single scan over all depths would take (lowest k on ties); a best sample sitting on a segment edge
+// takes its missing neighbour from the adjacent segment's first / last |F|^2.  One thread per pixel.
+__global__ void __launch_bounds__(256) peaks_combine_kernel(
+    const float* __restrict__ rec, int n_seg, long long n_pix, int n_phi, const float* __restrict__ phif,
+    double lambda0_sq, float* amp, float* phi, float* pa0, float* paz, int* idx) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pix) return;
+    PeakState s;
+    s.init();
+    float last = -1.f;
+    bool need_next = false;
+    for (int g = 0; g < n_seg; ++g) {
+        const float* r = rec + (long long)g * kPeakFields * n_pix + p;
+        const float first = r[6 * n_pix];
+        if (first == -1.f) continue;                       // empty segment (ragged last depth tile)
+        if (need_next) { s.best_yp2 = first; need_next = false; }
+        const float by2 = r[0];
+        if (by2 > s.best_y2) {
+            s.best_y2 = by2;
+            s.best_k = __float_as_int(r[1 * n_pix]);
+            s.best_q = r[2 * n_pix];
+            s.best_u = r[3 * n_pix];
+            const float ym2 = r[4 * n_pix], yp2 = r[5 * n_pix];
+            s.best_ym2 = ym2 == -1.f ? last : ym2;         // -1: the best was the segment's first sample
+            s.best_yp2 = yp2;
+            need_next = yp2 == -1.f;                       // -1: the best was the segment's last sample
+        }
+        last = r[7 * n_pix];
+    }
+    refine_and_store(s, n_phi, phif, lambda0_sq, p, amp, phi, pa0, paz, idx);
+}
+
+rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,
+                             float* pa0, float* paz, int* idx, cudaStream_t st) {
+    if (n_pix == 0) return RMSYNTH_OK;
+    peaks_combine_kernel<<<(unsigned)((n_pix + 255) / 256), 256, 0, st>>>(rec, n_seg, n_pix, p->n_phi, p->d_phif,
+                                                                           p->lambda0_sq, amp, phi, pa0, paz, idx);
+    RMS_LAUNCH_CHECK("peaks_combine_kernel");
+    return RMSYNTH_OK;
+}
+
+// |F| cube (Eq. 17) from FQ/FU cubes, element-wise (used by the FP32 comparison schemes; the tensor
+// kernel writes |F| from its epilogue registers).
+__global__ void __launch_bounds__(256) abs_cube_kernel(const float* __restrict__ FQ, const float* __restrict__ FU,
+                                                       long long n, float* __restrict__ FA) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float q = FQ[i], u = FU[i];
+        FA[i] = sqrtf(fmaf(q, q, u * u));
+    }
+}
+
+rmsynth_status abs_from_cubes(const float* FQ, const float* FU, long long n, float* FA, cudaStream_t st) {
+    if (n == 0) return RMSYNTH_OK;
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    abs_cube_kernel<<<(unsigned)blocks, 256, 0, st>>>(FQ, FU, n, FA);
+    RMS_LAUNCH_CHECK("abs_cube_kernel");
+    return RMSYNTH_OK;
 }
 
 rmsynth_status peaks_from_cubes(const rmsynth_plan* p, const float* FQ, const float* FU, long long n_pix,

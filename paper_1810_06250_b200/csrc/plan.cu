@@ -32,6 +32,27 @@ rmsynth_status ensure_scratch(const rmsynth_plan* p, int slot, size_t bytes, flo
     return RMSYNTH_OK;
 }
 
+rmsynth_status stream_scratch(const rmsynth_plan* p, cudaStream_t st, int tag, size_t bytes, float** out) {
+    std::lock_guard<std::mutex> g(p->pool_mu);
+    rmsynth_plan::StreamScratch* e = nullptr;
+    for (auto& x : p->pool)
+        if (x.st == st && x.tag == tag) e = &x;
+    if (!e) {
+        p->pool.push_back({st, tag, nullptr, 0});
+        e = &p->pool.back();
+    }
+    if (e->bytes < bytes) {
+        // the old buffer may still be in use by work already enqueued on this stream
+        if (e->ptr) { RMS_CUDA(cudaStreamSynchronize(st)); cudaFree(e->ptr); }
+        e->ptr = nullptr;
+        e->bytes = 0;
+        RMS_CUDA(cudaMalloc(&e->ptr, bytes));
+        e->bytes = bytes;
+    }
+    *out = e->ptr;
+    return RMSYNTH_OK;
+}
+
 // ---- a2: one thread per (channel i, depth k).  theta and its sincos are formed in FP64
 // (max|theta| reaches 713 rad in config 5; an FP32 theta would already miss the 1e-5 budget)
 // and only the product K w_i cos/sin is rounded to FP32.
@@ -227,6 +248,8 @@ rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
         if (q) cudaFree(q);
     for (int i = 0; i < rmsynth_plan::kScratch; ++i)
         if (p->scratch[i]) cudaFree(p->scratch[i]);
+    for (auto& x : p->pool)
+        if (x.ptr) cudaFree(x.ptr);
     for (int i = 0; i < 2; ++i)
         if (p->hs[i]) cudaStreamDestroy(p->hs[i]);
     delete p;

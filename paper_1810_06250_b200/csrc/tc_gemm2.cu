@@ -20,6 +20,7 @@
 #include <cstdlib>
 #include "common.cuh"
 #include "tc_common.cuh"
+#include "tc_epilogue.cuh"
 
 namespace rms {
 
@@ -33,20 +34,23 @@ constexpr int T2_STAGE = 4 * T2_APART + 2 * T2_BPART_MAX;   // 32 KB
 constexpr int T2_STAGES_PHI = 7, T2_STAGES_LOS = 6;
 constexpr int T2_SMEM = T2_STAGES_PHI * T2_STAGE + 2048;
 constexpr int T2_THREADS = 512;
-constexpr int T2_CHUNK_STAGES = 4;              // 32 channels per accumulator drain
+constexpr int T2_CHUNK_STAGES = 8;              // 64 channels per accumulator drain
 
-// Plan time: per (depth tile j, stage s, CTA rank): [part hi|lo][slot0 | slot1][row r < n][8 channels]
-//   rank 0: slot0 = Bc, slot1 = Bs;   rank 1: slot0 = -Bs, slot1 = Bc   (FP64 sincos, a2)
+// Plan time (a2): per (depth tile j, stage s, CTA rank): [part hi|lo][slot0 | slot1][row < n][8 channels].
+// slot0 feeds the Q MMAs, slot1 the U MMAs; each rank holds n of the 2n accumulator columns.  Column order
+// (tc_epilogue.cuh): depth d of the tile -> FQ column cq = (d/8)*16 + d%8, FU column cu = cq + 8, and
+//   FQ = Q.Bc + U.Bs,  FU = U.Bc - Q.Bs   =>   slot0[cq] = Bc, slot0[cu] = -Bs, slot1[cq] = Bs, slot1[cu] = Bc
+// Values are formed in FP64 (sincos of the FP64 phase) and split hi/lo at TF32 precision.
 __global__ void tc2_build_b_kernel(const double* __restrict__ delta, const double* __restrict__ kw,
                                    const double* __restrict__ phi, int n_chan, int n_phi, int n, int n_stages,
                                    float* __restrict__ blob) {
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;   // depth within the tile
     const int s = blockIdx.y, j = blockIdx.z;
-    if (r >= n) return;
-    const int k_phi = j * n + r;
+    if (d >= n) return;
+    const int k_phi = j * n + d;
     const size_t part = (size_t)2 * n * T2_KS;            // floats per split part
-    float* base0 = blob + (((size_t)j * n_stages + s) * 2 + 0) * 2 * part;
-    float* base1 = base0 + 2 * part;
+    float* base = blob + ((size_t)j * n_stages + s) * 2 * 2 * part;   // [rank][part][slot][row][8]
+    const int cq = (d >> 3) * 16 + (d & 7), cu = cq + 8;
     for (int k = 0; k < T2_KS; ++k) {
         const int i = s * T2_KS + k;
         double c = 0.0, sn = 0.0;
@@ -57,13 +61,18 @@ __global__ void tc2_build_b_kernel(const double* __restrict__ delta, const doubl
         }
         const float chi = rn_tf32((float)c), shi = rn_tf32((float)sn);
         const float clo = rn_tf32((float)(c - (double)chi)), slo = rn_tf32((float)(sn - (double)shi));
-        auto off = [&](int row) {   // SWIZZLE_32B K-major: 16-byte chunk index ^= bit 2 of the row
-            return ((size_t)row * T2_ROW + (((k / 4) ^ ((row >> 2) & 1)) * 16) + (k % 4) * 4) / 4;
+        auto put = [&](int col, int slot, float hi, float lo) {
+            const int rank = col >= n, row = col - rank * n + slot * n;
+            // SWIZZLE_32B K-major: 16-byte chunk index ^= bit 2 of the row
+            const size_t off = ((size_t)row * T2_ROW + (((k / 4) ^ ((row >> 2) & 1)) * 16) + (k % 4) * 4) / 4;
+            float* b = base + (size_t)rank * 2 * part;
+            b[off] = hi;
+            b[part + off] = lo;
         };
-        base0[off(r)] = chi;            base0[part + off(r)] = clo;            // rank 0 slot0: Bc
-        base0[off(n + r)] = shi;        base0[part + off(n + r)] = slo;        // rank 0 slot1: Bs
-        base1[off(r)] = -shi;           base1[part + off(r)] = -slo;           // rank 1 slot0: -Bs
-        base1[off(n + r)] = chi;        base1[part + off(n + r)] = clo;        // rank 1 slot1: Bc
+        put(cq, 0, chi, clo);
+        put(cu, 0, -shi, -slo);
+        put(cq, 1, shi, slo);
+        put(cu, 1, chi, clo);
     }
 }
 
@@ -71,8 +80,10 @@ struct Tc2Params {
     long long n_pix;
     int n_chan, n_phi, n, n_phi_tiles, n_stages, n_items, a3d;
     const float* blob;
-    float* FQ;
+    float* FQ;           // may be NULL (maps only)
     float* FU;
+    float* FA;           // |F| cube (Eq. 17), may be NULL
+    float* rec;          // peak-segment records (tc_epilogue.cuh), NULL = no peak search
     long long* prof;
 };
 
@@ -194,8 +205,8 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
             if (prof) {
-                prm.prof[cluster_id * 4 + 0] = 0; prm.prof[cluster_id * 4 + 1] = w_ready;
-                prm.prof[cluster_id * 4 + 2] = w_acc; prm.prof[cluster_id * 4 + 3] = clock64() - t_begin;
+                prm.prof[cluster_id * 8 + 0] = 0; prm.prof[cluster_id * 8 + 1] = w_ready;
+                prm.prof[cluster_id * 8 + 2] = w_acc; prm.prof[cluster_id * 8 + 3] = clock64() - t_begin;
             }
         }
         __syncwarp();
@@ -234,12 +245,15 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         uint32_t ab = 0, aph = 0;
         float acc[128];
+        const bool prof = prm.prof != nullptr && warp == 8 && rank == 0;
+        long long e_wait = 0, e_drain = 0, e_store = 0, e_scan = 0, t0 = 0, t1 = 0;
         for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
             const int tp = item / prm.n_phi_tiles, j = item - tp * prm.n_phi_tiles;
             const long long P0 = (long long)(2 * tp + (int)rank) * T2_M + q * 32;   // first pixel of this warp
-            const long long p = P0 + lane;
             for (int c = 0; c < n_chunks; ++c) {
+                if (prof) t0 = clock64();
                 mbar_wait(&acc_full[ab], aph);
+                if (prof) { t1 = clock64(); e_wait += t1 - t0; }
                 tc_fence_after();
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
@@ -260,49 +274,30 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(mapa_u32(smem_u32(&acc_empty[ab]), 0));
                 if (++ab == 2) { ab = 0; aph ^= 1; }
+                if (prof) e_drain += clock64() - t1;
             }
-            const int nv = min(n, prm.n_phi - j * n);
-            const int q_end = nv - cbase, u_beg = n - cbase, u_end = n + nv - cbase;
-            const long long kq = (long long)j * n + cbase, ku = kq - n;
-            if (!OUT_LOS) {
-                if (p < prm.n_pix) {
-                    const long long sb = 4LL * prm.n_pix;
-                    unsigned long long aq = (unsigned long long)(prm.FQ + kq * prm.n_pix + p);
-                    unsigned long long au = (unsigned long long)(prm.FU + ku * prm.n_pix + p);
-                    asm volatile("" : "+l"(aq), "+l"(au));
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) {
-                        if (g * 32 < q_end) {
-#pragma unroll
-                            for (int i = g * 32; i < g * 32 + 32; ++i) st_global_pred(aq + i * sb, acc[i], i < q_end);
-                        }
-                        if (g * 32 + 32 > u_beg && g * 32 < u_end) {
-#pragma unroll
-                            for (int i = g * 32; i < g * 32 + 32; ++i)
-                                st_global_pred(au + i * sb, acc[i], (unsigned)(i - u_beg) < (unsigned)nv);
-                        }
-                    }
-                }
+            if (prof) t0 = clock64();
+            EpiTile et;
+            et.n_pix = prm.n_pix;
+            et.P0 = P0;
+            et.n_phi = prm.n_phi;
+            et.k0 = j * n + (cbase >> 1);
+            et.nv = min(n, prm.n_phi - j * n) - (cbase >> 1);
+            et.seg = 2 * j + (cbase >> 7);
+            float* sT = stage_t + (warp - 8) * (32 * 33);
+            if (prm.rec) {
+                if (!OUT_LOS) epi_tile_phi_major<true>(acc, et, lane, prm.FQ, prm.FU, prm.FA, prm.rec);
+                else epi_tile_los_major<true>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, prm.rec);
             } else {
-                float* sT = stage_t + (warp - 8) * (32 * 33);
-                const int rows = (int)max(0LL, min(32LL, prm.n_pix - P0));
-                const long long rb = 4LL * prm.n_phi;
-#pragma unroll
-                for (int g = 0; g < 4; ++g) {
-                    const int i = g * 32 + lane;
-                    const bool is_q = i < q_end, is_u = (unsigned)(i - u_beg) < (unsigned)nv;
-                    if (g * 32 < q_end || (g * 32 + 32 > u_beg && g * 32 < u_end)) {
-#pragma unroll
-                        for (int c = 0; c < 32; ++c) sT[lane * 33 + c] = acc[g * 32 + c];
-                        __syncwarp();
-                        unsigned long long a = (unsigned long long)((is_u ? prm.FU + ku : prm.FQ + kq) + P0 * prm.n_phi + i);
-#pragma unroll 8
-                        for (int r = 0; r < 32; ++r)
-                            st_global_pred(a + r * rb, sT[r * 33 + lane], (is_q || is_u) && r < rows);
-                        __syncwarp();
-                    }
-                }
+                if (!OUT_LOS) epi_tile_phi_major<false>(acc, et, lane, prm.FQ, prm.FU, prm.FA, nullptr);
+                else epi_tile_los_major<false>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, nullptr);
             }
+            if (prof) { t1 = clock64(); e_store += t1 - t0; }
+            if (prof) e_scan += clock64() - t1;
+        }
+        if (prof && lane == 0) {
+            prm.prof[cluster_id * 8 + 4] = e_wait; prm.prof[cluster_id * 8 + 5] = e_drain;
+            prm.prof[cluster_id * 8 + 6] = e_store; prm.prof[cluster_id * 8 + 7] = e_scan;
         }
     }
     tc_fence_before();
@@ -327,7 +322,7 @@ rmsynth_status tc2_plan_init(rmsynth_plan* p) {
 }
 
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, cudaStream_t st) {
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st) {
     Tc2Params prm;
     prm.n_pix = n_pix;
     prm.n_chan = p->n_chan;
@@ -341,14 +336,16 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.blob = p->d_tcB2;
     prm.FQ = FQ;
     prm.FU = FU;
+    prm.FA = FA;
+    prm.rec = rec;
     prm.prof = nullptr;
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
     const int grid = 2 * clusters;
     static const bool want_prof = getenv("RMSYNTH_TC_PROFILE") != nullptr;
     if (want_prof) {
-        RMS_CUDA(cudaMalloc(&prm.prof, sizeof(long long) * 4 * clusters));
-        RMS_CUDA(cudaMemset(prm.prof, 0, sizeof(long long) * 4 * clusters));
+        RMS_CUDA(cudaMalloc(&prm.prof, sizeof(long long) * 8 * clusters));
+        RMS_CUDA(cudaMemset(prm.prof, 0, sizeof(long long) * 8 * clusters));
     }
     const CUtensorMap& mq = *static_cast<const CUtensorMap*>(map_q);
     const CUtensorMap& mu = *static_cast<const CUtensorMap*>(map_u);
@@ -358,13 +355,14 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     else tc2_rmsynth_kernel<0, 1><<<grid, T2_THREADS, T2_SMEM, st>>>(mq, mu, prm);
     RMS_LAUNCH_CHECK("tc2_rmsynth_kernel");
     if (want_prof) {   // debug only: synchronises
-        std::vector<long long> h(4 * clusters);
-        RMS_CUDA(cudaMemcpy(h.data(), prm.prof, sizeof(long long) * 4 * clusters, cudaMemcpyDeviceToHost));
+        std::vector<long long> h(8 * clusters);
+        RMS_CUDA(cudaMemcpy(h.data(), prm.prof, sizeof(long long) * 8 * clusters, cudaMemcpyDeviceToHost));
         cudaFree(prm.prof);
-        double a[4] = {0, 0, 0, 0};
-        for (int i = 0; i < clusters; ++i) for (int j = 0; j < 4; ++j) a[j] += (double)h[4 * i + j] / clusters;
-        fprintf(stderr, "[rmsynth tc2 profile] MMA thread: total %.0f cyc; waiting ready %.1f%% acc_empty %.1f%%\n", a[3],
-                100 * a[1] / a[3], 100 * a[2] / a[3]);
+        double a[8] = {};
+        for (int i = 0; i < clusters; ++i) for (int j = 0; j < 8; ++j) a[j] += (double)h[8 * i + j] / clusters;
+        fprintf(stderr, "[rmsynth tc2 profile] MMA thread: total %.0f cyc; waiting ready %.1f%% acc_empty %.1f%% | epilogue warp: "
+                "wait %.1f%% drain %.1f%% store %.1f%% scan %.1f%%\n", a[3], 100 * a[1] / a[3], 100 * a[2] / a[3],
+                100 * a[4] / a[3], 100 * a[5] / a[3], 100 * a[6] / a[3], 100 * a[7] / a[3]);
     }
     return RMSYNTH_OK;
 }

@@ -196,6 +196,51 @@ def test_peak_refinement_on_nonuniform_grid_and_edges(b, oracle_mod):
         plan.destroy()
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("lin,lout", LAYOUTS)
+def test_abs_cube_and_maps_only(b, oracle_mod, scheme, lin, lout):
+    """rmsynth_execute_ex: the |F| cube (Eq. 17) alone, with the cubes, and maps without any cube.
+    Shapes chosen so that depth tiles are ragged (n_phi = 401 -> 4 tiles of 104, second warp half 40 wide)."""
+    cfg, nu, w, phi, q, u = inputs(5, 389, start=3)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    Fabs = np.sqrt(FQ ** 2 + FU ** 2)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    n_pix, n_phi = q.shape[0], plan.n_phi
+    layout = (b.IN_FREQ_MAJOR if lin == "freq" else 0) | (b.OUT_PHI_MAJOR if lout == "phi" else 0)
+    dq = torch.from_numpy(q if lin == "los" else np.ascontiguousarray(q.T)).cuda()
+    du = torch.from_numpy(u if lin == "los" else np.ascontiguousarray(u.T)).cuda()
+    shape = (n_pix, n_phi) if lout == "los" else (n_phi, n_pix)
+    new = lambda: torch.full(shape, float("nan"), device="cuda")
+    los = lambda t: t.cpu().numpy() if lout == "los" else t.cpu().numpy().T
+    fa = new()
+    plan.execute_ex(dq, du, n_pix, layout, F_abs=fa)                       # |F| cube only
+    torch.cuda.synchronize()
+    assert np.all(np.abs(los(fa) - Fabs) <= 1.5 * TOL * T[:, None]), "F_abs alone"
+    fq, fu, fa2 = new(), new(), new()
+    maps = {k: torch.full((n_pix,), float("nan"), device="cuda") for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero")}
+    maps["peak_index"] = torch.full((n_pix,), -1, dtype=torch.int32, device="cuda")
+    plan.execute_ex(dq, du, n_pix, layout, FQ=fq, FU=fu, F_abs=fa2, **maps)
+    torch.cuda.synchronize()
+    check_cubes(los(fq), los(fu), FQ, FU, T, "execute_ex cubes")
+    assert torch.equal(fa, fa2)
+    assert torch.equal(fa2, torch.sqrt(torch.addcmul(fu * fu, fq, fq))) or \
+        float((fa2 - torch.sqrt(fq * fq + fu * fu)).abs().max()) <= 2e-7 * float(fa2.max())
+    got = {("kstar" if k == "peak_index" else k): v.cpu().numpy() for k, v in maps.items()}
+    check_peaks(oracle_mod, op, FQ, FU, T, got, cfg.dphi, f"execute_ex {scheme}")
+    # the arg-max the fused epilogue takes must be the arg-max of the |F|^2 it could form from its own cube
+    y2 = torch.addcmul(fu * fu, fq, fq) if False else (fq * fq + fu * fu)
+    km = y2.argmax(1 if lout == "los" else 0).cpu().numpy()
+    ymax = y2.amax(1 if lout == "los" else 0).cpu().numpy()
+    ysel = (y2 if lout == "los" else y2.T)[torch.arange(n_pix), torch.as_tensor(got["kstar"], device="cuda").long()].cpu().numpy()
+    assert np.all(ysel >= ymax * (1 - 3e-7)), "fused arg-max is not the maximum of the written cube"
+    maps2 = {k: torch.full_like(v, -1) for k, v in maps.items()}
+    plan.execute_ex(dq, du, n_pix, layout, **maps2)                        # maps only: no cube is written
+    torch.cuda.synchronize()
+    for k in maps:
+        assert torch.equal(maps[k], maps2[k]), k
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ host streaming + API edges
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("lin,lout", [("freq", "phi"), ("los", "los"), ("freq", "los")])
