@@ -54,6 +54,9 @@ enum {
     RMSYNTH_SCHEME_AUTO = 0,        /* = 3xTF32 tensor cores                             */
     RMSYNTH_SCHEME_TF32X3 = 1,      /* tcgen05 tensor cores, split-precision 3xTF32,     */
                                     /* FP32 accumulate in TMEM                           */
+    RMSYNTH_SCHEME_F16X3 = 2,       /* tcgen05 tensor cores, block-scaled FP16 hi/lo split    */
+                                    /* (3 products at twice the TF32 rate), FP32 accumulate;  */
+                                    /* zero-weight channels are ignored even if non-finite    */
     RMSYNTH_SCHEME_FP32_TABLE = 3,  /* CUDA cores, FP32 FMA, reads the plan's cos/sin    */
     RMSYNTH_SCHEME_FP32_SINCOS = 4  /* CUDA cores, sincos on the fly, one (pixel,phi)    */
                                     /* per thread -- the paper's kernel shape    */

@@ -19,7 +19,7 @@ _lib = C.CDLL(LIB_PATH)
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
 IN_LOS_MAJOR, IN_FREQ_MAJOR, OUT_LOS_MAJOR, OUT_PHI_MAJOR = 0, 1, 0, 2
-SCHEME_AUTO, SCHEME_TF32X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS = 0, 1, 3, 4
+SCHEME_AUTO, SCHEME_TF32X3, SCHEME_F16X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS = 0, 1, 2, 3, 4
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
            "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_rmsf",

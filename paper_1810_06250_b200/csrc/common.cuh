@@ -63,6 +63,11 @@ struct rmsynth_plan {
     // tensor path (tc_gemm.cu)
     rms::TcGeom tc;
     float* d_tcB2 = nullptr;              // pre-split, pre-swizzled B operand blobs (tc_gemm2.cu)
+    // FP16 split tensor path (tc_gemm3.cu)
+    rms::TcGeom tc3;
+    void* d_tcB3 = nullptr;               // scaled FP16 hi/lo B operand blobs
+    unsigned int* d_tc3mask = nullptr;    // per 32-channel chunk: channels with w > 0
+    int tc3_eb = 0;                       // B is scaled by 2^tc3_eb
     void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
@@ -100,6 +105,11 @@ void tc_plan_free(rmsynth_plan* p);
 rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
                           float* FQ, float* FU, float* FA, float* amp, float* phi, float* pa0, float* paz, int* idx,
                           cudaStream_t st);
+
+// tc_gemm3.cu
+rmsynth_status tc3_plan_init(rmsynth_plan* p);
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st);
 
 // tc_gemm2.cu
 rmsynth_status tc2_plan_init(rmsynth_plan* p);

@@ -31,7 +31,7 @@ static rmsynth_status check_args(const rmsynth_plan* p, const float* Q, const fl
 // Device-resident contraction + optional |F| cube and maps on one stream; never synchronises.
 static rmsynth_status run_device(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
                                  Outs o, cudaStream_t st) {
-    if (p->scheme == RMSYNTH_SCHEME_TF32X3)
+    if (p->scheme == RMSYNTH_SCHEME_TF32X3 || p->scheme == RMSYNTH_SCHEME_F16X3)
         return tc_execute(p, Q, U, n_pix, layout, o.FQ, o.FU, o.FA, o.amp, o.phi, o.pa0, o.paz, o.idx, st);
     // FP32 CUDA-core comparison paths: cubes first, then the stand-alone |F| and peak kernels.
     rmsynth_status s;

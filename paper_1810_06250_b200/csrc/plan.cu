@@ -148,7 +148,7 @@ static rmsynth_status build_plan(rmsynth_plan* p) {
     p->R_re.resize(np);
     p->R_im.resize(np);
     if ((st = device_rmsf(p, p->d_phi, np, p->R_re.data(), p->R_im.data()))) return st;
-    if (p->scheme == RMSYNTH_SCHEME_TF32X3 && (st = tc_plan_init(p))) return st;
+    if ((p->scheme == RMSYNTH_SCHEME_TF32X3 || p->scheme == RMSYNTH_SCHEME_F16X3) && (st = tc_plan_init(p))) return st;
     RMS_CUDA(cudaDeviceSynchronize());
     return RMSYNTH_OK;
 }
@@ -174,7 +174,7 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
         std::memcpy(&o, opt, opt->struct_size);
     }
     int scheme = o.scheme == RMSYNTH_SCHEME_AUTO ? RMSYNTH_SCHEME_TF32X3 : o.scheme;
-    if (scheme != RMSYNTH_SCHEME_TF32X3 && scheme != RMSYNTH_SCHEME_FP32_TABLE && scheme != RMSYNTH_SCHEME_FP32_SINCOS)
+    if (scheme != RMSYNTH_SCHEME_TF32X3 && scheme != RMSYNTH_SCHEME_F16X3 && scheme != RMSYNTH_SCHEME_FP32_TABLE && scheme != RMSYNTH_SCHEME_FP32_SINCOS)
         return fail(RMSYNTH_EINVAL, "unknown scheme");
     if (o.lambda0_mode < 0 || o.lambda0_mode > 2) return fail(RMSYNTH_EINVAL, "unknown lambda0_mode");
     if (o.lambda0_mode == 2 && !std::isfinite(o.lambda0_sq)) return fail(RMSYNTH_EINVAL, "lambda0_sq not finite");

@@ -44,12 +44,16 @@ rmsynth_status tc_plan_init(rmsynth_plan* p) {
     g.k_pad = n_stages * TC_KS;
     g.ctas = 2;
     if (!get_encode_fn()) return fail(RMSYNTH_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-    return tc2_plan_init(p);
+    return p->scheme == RMSYNTH_SCHEME_F16X3 ? tc3_plan_init(p) : tc2_plan_init(p);
 }
 
 void tc_plan_free(rmsynth_plan* p) {
     if (p->d_tcB2) cudaFree(p->d_tcB2);
+    if (p->d_tcB3) cudaFree(p->d_tcB3);
+    if (p->d_tc3mask) cudaFree(p->d_tc3mask);
     p->d_tcB2 = nullptr;
+    p->d_tcB3 = nullptr;
+    p->d_tc3mask = nullptr;
 }
 
 // Copy a cube into a buffer whose row pitch is a multiple of 4 floats (TMA needs 16-byte strides).
@@ -62,13 +66,13 @@ __global__ void tc_repack_kernel(const float* __restrict__ src, float* __restric
 }
 
 static rmsynth_status make_map3(CUtensorMap* m, const float* base, uint64_t n_chan, uint64_t n_pix, uint64_t pitch_floats,
-                                uint32_t ks) {
+                                uint32_t ks, CUtensorMapSwizzle sw = CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B) {
     cuuint64_t dims[3] = {32, n_chan, n_pix / 32};
     cuuint64_t strides[2] = {pitch_floats * 4, 128};
     cuuint32_t box[3] = {32, ks, 4};
     cuuint32_t es[3] = {1, 1, 1};
     CUresult r = get_encode_fn()(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides, box, es,
-                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(RMSYNTH_ECUDA, "cuTensorMapEncodeTiled(3d) failed with code " + std::to_string((int)r));
     return RMSYNTH_OK;
@@ -114,27 +118,34 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     }
     CUtensorMap mq, mu_;
     const bool a3d = in_freq && (n_pix % 32 == 0);
+    const bool f16 = p->scheme == RMSYNTH_SCHEME_F16X3;
+    // channels per TMA box: one 8-channel MMA stage (3xTF32) or one 32-channel chunk (FP16 split, raw tile)
+    const uint32_t kbox = f16 ? 32 : TC_KS;
+    const CUtensorMapSwizzle sw_mn = f16 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
+    const CUtensorMapSwizzle sw_k = f16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_32B;
     if (a3d) {
-        if ((s = make_map3(&mq, Q, p->n_chan, n_pix, pitch, TC_KS)) || (s = make_map3(&mu_, U, p->n_chan, n_pix, pitch, TC_KS)))
+        if ((s = make_map3(&mq, Q, p->n_chan, n_pix, pitch, kbox, sw_mn)) || (s = make_map3(&mu_, U, p->n_chan, n_pix, pitch, kbox, sw_mn)))
             return s;
     } else if (in_freq) {
-        if ((s = make_map(&mq, Q, n_pix, p->n_chan, pitch, 32, TC_KS, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)) ||
-            (s = make_map(&mu_, U, n_pix, p->n_chan, pitch, 32, TC_KS, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)))
+        if ((s = make_map(&mq, Q, n_pix, p->n_chan, pitch, 32, kbox, sw_mn)) ||
+            (s = make_map(&mu_, U, n_pix, p->n_chan, pitch, 32, kbox, sw_mn)))
             return s;
     } else {
-        if ((s = make_map(&mq, Q, p->n_chan, n_pix, pitch, TC_KS, TC_M, CU_TENSOR_MAP_SWIZZLE_32B)) ||
-            (s = make_map(&mu_, U, p->n_chan, n_pix, pitch, TC_KS, TC_M, CU_TENSOR_MAP_SWIZZLE_32B)))
+        if ((s = make_map(&mq, Q, p->n_chan, n_pix, pitch, kbox, TC_M, sw_k)) ||
+            (s = make_map(&mu_, U, p->n_chan, n_pix, pitch, kbox, TC_M, sw_k)))
             return s;
     }
     // Fused peak search (a7): the epilogue warps write one record per (pixel, 64-depth segment); a small
     // second kernel merges a pixel's segments and refines.  No cube is re-read, none is needed (maps only).
     float* rec = nullptr;
-    const int n_seg = 2 * p->tc.n_phi_tiles;
+    const int n_seg = 2 * (f16 ? p->tc3.n_phi_tiles : p->tc.n_phi_tiles);
     if (want_maps) {
         size_t bytes = sizeof(float) * 8 * (size_t)n_seg * (size_t)n_pix;
         if ((s = stream_scratch(p, st, SCR_PEAK_REC, bytes, &rec))) return s;
     }
-    if ((s = tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, st))) return s;
+    s = f16 ? tc3_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, st)
+            : tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, st);
+    if (s) return s;
     if (!want_maps) return RMSYNTH_OK;
     return peaks_combine(p, rec, n_seg, n_pix, amp, phi, pa0, paz, idx, st);
 }

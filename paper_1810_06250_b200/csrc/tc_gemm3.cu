@@ -1,0 +1,458 @@
+// Rows a4-a8, scheme FP16X3: the contraction of Eqs. 15-16 on tcgen05 tensor cores with a
+// block-scaled FP16 split, twice the tensor rate of the 3xTF32 scheme (tc_gemm2.cu) at the same accuracy.
+//
+//   [FQ | FU](256 pixels x 2n depths)  =  Q [Bc | -Bs]  +  U [Bs | Bc],   per CTA pair (cta_group::2, M = 256)
+//
+// Split precision.  kind::f16 multiplies 11-bit significands exactly and honours FP16 subnormals (measured,
+// profiles/r01_probe_f16.txt), so a value scaled into [2^14, 2^15) is carried as hi + lo (two FP16 numbers,
+// 22 significant bits, absolute floor 2^-25): x s = hi + lo,  F = sum (hi_a hi_b + lo_a hi_b + hi_a lo_b).
+//   * B = K w cos/sin is scaled once at plan time by a power of two (FP64 split).
+//   * Q, U are scaled per (pixel, 32-channel chunk) by a power of two taken from the chunk's largest |sample|
+//     over the channels with w > 0; zero-weight channels are replaced by zeros (they contribute nothing, A13),
+//     so a flagged channel full of interference cannot crush the scale of its neighbours.
+//   * The TMEM FP32 accumulator is drained after every chunk (12 MMAs) into FP32 registers with
+//     acc += drained * 2^-e(pixel, chunk): the drains the accumulator's round-toward-zero already demands
+//     (tc_gemm2.cu) are what makes a per-chunk scale free.
+// A operands never touch shared memory as MMA operands: the transform warps convert the raw TMA tile in
+// registers and write hi/lo straight into TENSOR MEMORY (tcgen05.st); the MMAs take A from TMEM (".ts" form).
+// Shared memory carries only the raw FP32 tile (written by TMA, read once) and the B operand.
+//
+// TMEM (512 columns): accumulator buffers at columns 0 and 208 (2n <= 208 columns each), A ring of three
+// 16-channel slots at 416 + 32 s: [Q_hi 8 | Q_lo 8 | U_hi 8 | U_lo 8] columns, two FP16 per column.
+//
+// Warps (512 threads, 1 CTA/SM, CTA pairs, persistent over (pixel-tile pair, depth tile) items):
+//   0 raw-tile TMA producer | 1 MMA issuer (leader CTA) | 2 TMEM allocator + B producer | 4-7 transform |
+//   8-15 epilogue (tc_epilogue.cuh: stores in either layout, |F| cube, fused peak search)
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <cstdio>
+#include <cstdlib>
+#include "common.cuh"
+#include "tc_common.cuh"
+#include "tc_epilogue.cuh"
+
+namespace rms {
+
+constexpr int T3_M = 128;                        // pixels per CTA (UMMA M = 256 per pair)
+constexpr int T3_NMAX = 104;                     // depths per tile: 2 x 2n accumulator columns + 96 A columns = 512
+constexpr int T3_KC = 32;                        // channels per chunk (scale and drain granularity)
+constexpr int T3_RAW = 2 * T3_M * T3_KC * 4;     // 32 KB: raw Q tile + raw U tile of one chunk
+constexpr int T3_BSTAGE = 256 * T3_NMAX;         // 26 KB: [hi|lo][slot0|slot1][4 k-cores][n rows][8 halves]
+constexpr int T3_R = 3, T3_S = 3, T3_NA = 3;     // raw ring, B ring (chunks); A ring in TMEM (16-channel slots)
+constexpr int T3_SCALES = 8;                     // ring of per-pixel chunk scales (transform -> epilogue)
+constexpr int T3_ACC_COLS = 208, T3_A_COL0 = 416;
+constexpr int T3_OFF_B = T3_R * T3_RAW;
+constexpr int T3_OFF_SCALE = T3_OFF_B + T3_S * T3_BSTAGE;
+constexpr int T3_OFF_BARS = T3_OFF_SCALE + T3_SCALES * T3_M * 4;
+constexpr int T3_OFF_STAGE_T = T3_OFF_BARS + 512;
+constexpr int T3_SMEM_PHI = T3_OFF_STAGE_T + 1024;                    // + alignment slack
+constexpr int T3_SMEM_LOS = T3_OFF_STAGE_T + 8 * 32 * 33 * 4 + 1024;
+constexpr int T3_THREADS = 512;
+static_assert(T3_SMEM_LOS <= 227 * 1024, "shared memory budget");
+
+__device__ __forceinline__ void umma2_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}" ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc),
+        "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------------
+// Plan time (a2): the scaled FP16 hi/lo B operand.  One blob per (depth tile j, chunk c, CTA rank):
+//   [part hi|lo][slot0 | slot1][k-core kc < 4][row < n][8 channels]   (no-swizzle K-major core matrices)
+// slot0 feeds the Q MMAs, slot1 the U MMAs; accumulator column order as in tc_epilogue.cuh:
+//   depth d -> FQ column cq = (d/8)*16 + d%8, FU column cu = cq + 8;  rank r holds columns [r n, r n + n)
+//   slot0[cq] = Bc, slot0[cu] = -Bs, slot1[cq] = Bs, slot1[cu] = Bc.     Values: FP64 sincos, scaled by 2^eB.
+__global__ void tc3_build_b_kernel(const double* __restrict__ delta, const double* __restrict__ kw,
+                                   const double* __restrict__ phi, int n_chan, int n_phi, int n, int n_chunks,
+                                   double scale_b, __half* __restrict__ blob) {
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;   // depth within the tile
+    const int c = blockIdx.y, j = blockIdx.z;
+    if (d >= n) return;
+    const int k_phi = j * n + d;
+    const size_t rank_halves = (size_t)128 * n;           // 256 n bytes per rank
+    __half* base = blob + ((size_t)j * n_chunks + c) * 2 * rank_halves;
+    const int cq = (d >> 3) * 16 + (d & 7), cu = cq + 8;
+    for (int k = 0; k < T3_KC; ++k) {
+        const int i = c * T3_KC + k;
+        double cs = 0.0, sn = 0.0;
+        if (i < n_chan && k_phi < n_phi) {
+            sincos(2.0 * phi[k_phi] * delta[i], &sn, &cs);
+            cs *= kw[i] * scale_b;
+            sn *= kw[i] * scale_b;
+        }
+        const __half chi = __double2half(cs), shi = __double2half(sn);
+        const __half clo = __double2half(cs - (double)__half2float(chi)), slo = __double2half(sn - (double)__half2float(shi));
+        auto put = [&](int col, int slot, __half hi, __half lo) {
+            const int rank = col >= n, row = col - rank * n;
+            const size_t off = (size_t)rank * rank_halves + (size_t)slot * 32 * n + (size_t)(k >> 3) * 8 * n + (size_t)row * 8 + (k & 7);
+            base[off] = hi;
+            base[off + (size_t)64 * n] = lo;
+        };
+        put(cq, 0, chi, clo);
+        put(cu, 0, __hneg(shi), __hneg(slo));
+        put(cq, 1, shi, slo);
+        put(cu, 1, chi, clo);
+    }
+}
+
+struct Tc3Params {
+    long long n_pix;
+    int n_chan, n_phi, n, n_phi_tiles, n_chunks, n_items, a3d;
+    float inv_scale_b;            // 2^-eB
+    const __half* blob;
+    const uint32_t* chan_mask;    // [n_chunks] bit i: channel 32 c + i exists and has w > 0
+    float* FQ;                    // may be NULL
+    float* FU;
+    float* FA;                    // |F| cube, may be NULL
+    float* rec;                   // peak-segment records, NULL = no peak search
+};
+
+// ------------------------------------------------------------------------------------------------
+// Transform (a4): one thread per pixel row.  v[0..31] = Q, v[32..63] = U of the chunk's 32 channels.
+__device__ __forceinline__ void t3_load_raw(const uint8_t* raw, int row, bool in_mn, float (&v)[64]) {
+    if (in_mn) {        // [operand][pixel group][channel][32 pixels]: a warp reads 128 contiguous bytes per channel
+        const float* q = reinterpret_cast<const float*>(raw) + (row >> 5) * 1024 + (row & 31);
+#pragma unroll
+        for (int c = 0; c < 32; ++c) { v[c] = q[c * 32]; v[32 + c] = q[4096 + c * 32]; }
+    } else {            // [operand][pixel][32 channels], 128-byte rows, SWIZZLE_128B: 16-byte unit i sits at i ^ (row & 7)
+        const uint8_t* q = raw + row * 128;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int o = (i ^ (row & 7)) * 16;
+            const float4 a = *reinterpret_cast<const float4*>(q + o), b = *reinterpret_cast<const float4*>(q + 16384 + o);
+            v[4 * i] = a.x; v[4 * i + 1] = a.y; v[4 * i + 2] = a.z; v[4 * i + 3] = a.w;
+            v[32 + 4 * i] = b.x; v[32 + 4 * i + 1] = b.y; v[32 + 4 * i + 2] = b.z; v[32 + 4 * i + 3] = b.w;
+        }
+    }
+}
+
+// hi = t truncated to 11 significant bits (exact in FP16 unless subnormal there), lo = t - hi; two channels per register
+__device__ __forceinline__ void t3_split(float x0, float x1, float scale, uint32_t& hi, uint32_t& lo) {
+    const float t0 = x0 * scale, t1 = x1 * scale;
+    const float h0 = __uint_as_float(__float_as_uint(t0) & 0xFFFFE000u), h1 = __uint_as_float(__float_as_uint(t1) & 0xFFFFE000u);
+    const __half2 h = __floats2half2_rn(h0, h1), l = __floats2half2_rn(t0 - h0, t1 - h1);
+    hi = *reinterpret_cast<const uint32_t*>(&h);
+    lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
+template <int IN_MN, int OUT_LOS>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
+tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU, const Tc3Params prm) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    float* scales = reinterpret_cast<float*>(smem_gen + T3_OFF_SCALE);            // [T3_SCALES][128]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_gen + T3_OFF_BARS);
+    uint64_t* raw_full = bars;                    // [R] raw tile landed                     (1 + tx)
+    uint64_t* raw_empty = raw_full + T3_R;        // [R] raw tile read by the transform      (4 warps)
+    uint64_t* b_full = raw_empty + T3_R;          // [S] B chunk landed                      (1 + tx)
+    uint64_t* b_empty = b_full + T3_S;            // [S] MMAs of the chunk done, both CTAs   (multicast commit)
+    uint64_t* a_ready = b_empty + T3_S;           // [NA] LEADER's: slot written in both CTAs (4 local + 4 remote warps)
+    uint64_t* a_empty = a_ready + T3_NA;          // [NA] MMAs that read the slot done        (multicast commit)
+    uint64_t* acc_full = a_empty + T3_NA;         // [2] chunk accumulated, both CTAs         (multicast commit)
+    uint64_t* acc_empty = acc_full + 2;           // [2] LEADER's: chunk drained by both epilogues (8 + 8 warps)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+    float* stage_t = reinterpret_cast<float*>(smem_gen + T3_OFF_STAGE_T);         // LOS-major transpose buffers
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+    const int n = prm.n, N2 = 2 * prm.n;
+    const uint32_t b_bytes = 256u * n;
+    const int n_chunks = prm.n_chunks;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < T3_R; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], 4); }
+        for (int s = 0; s < T3_S; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 1); }
+        for (int s = 0; s < T3_NA; ++s) { mbar_init(&a_ready[s], 8); mbar_init(&a_empty[s], 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], 16); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp < 4) {
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+      if (warp == 0) {
+        // ===================== raw-tile TMA producer (both CTAs) =====================
+        if (lane == 0) {
+            uint32_t st = 0, ph = 0;
+            for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
+                const int tp = item / prm.n_phi_tiles;
+                const int pix0 = (2 * tp + (int)rank) * T3_M;       // may lie past n_pix: TMA zero-fills
+                for (int c = 0; c < n_chunks; ++c) {
+                    mbar_wait(&raw_empty[st], ph ^ 1);
+                    mbar_expect_tx(&raw_full[st], T3_RAW);
+                    const uint32_t sb = smem_base + st * T3_RAW;
+                    if (IN_MN) {
+                        if (prm.a3d) {   // one box per operand: 32 pixels x 32 channels x 4 pixel groups
+                            tma_load_3d(sb, &mapQ, 0, c * T3_KC, pix0 / 32, &raw_full[st]);
+                            tma_load_3d(sb + T3_RAW / 2, &mapU, 0, c * T3_KC, pix0 / 32, &raw_full[st]);
+                        } else {
+#pragma unroll
+                            for (int g = 0; g < 4; ++g) {
+                                tma_load_2d(sb + g * 4096, &mapQ, pix0 + 32 * g, c * T3_KC, &raw_full[st]);
+                                tma_load_2d(sb + T3_RAW / 2 + g * 4096, &mapU, pix0 + 32 * g, c * T3_KC, &raw_full[st]);
+                            }
+                        }
+                    } else {             // [pix][chan]: one box of 32 channels x 128 pixels per operand
+                        tma_load_2d(sb, &mapQ, c * T3_KC, pix0, &raw_full[st]);
+                        tma_load_2d(sb + T3_RAW / 2, &mapU, c * T3_KC, pix0, &raw_full[st]);
+                    }
+                    if (++st == T3_R) { st = 0; ph ^= 1; }
+                }
+            }
+        }
+        __syncwarp();
+      } else if (warp == 2) {
+        // ===================== B producer (both CTAs): one bulk copy per chunk =====================
+        if (lane == 0) {
+            uint32_t st = 0, ph = 0;
+            for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
+                const int j = item % prm.n_phi_tiles;
+                const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) + ((size_t)j * n_chunks * 2 + rank) * b_bytes;
+                for (int c = 0; c < n_chunks; ++c) {
+                    mbar_wait(&b_empty[st], ph ^ 1);
+                    mbar_expect_tx(&b_full[st], b_bytes);
+                    bulk_load(smem_base + T3_OFF_B + st * T3_BSTAGE, bsrc + (size_t)c * 2 * b_bytes, b_bytes, &b_full[st]);
+                    if (++st == T3_S) { st = 0; ph ^= 1; }
+                }
+            }
+        }
+        __syncwarp();
+      } else if (warp == 1) {
+        // ===================== MMA issuer (leader CTA only) =====================
+        if (lane == 0 && rank == 0) {
+            // kind::f16: D = F32 (bit 4), A = B = F16 (0), K-major, N = 2n, M = 256
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+            uint32_t sa = 0, pa = 0, sb = 0, pb = 0, ab = 0, aph = 0;
+            for (int item = cluster_id; item < prm.n_items; item += n_clusters)
+                for (int c = 0; c < n_chunks; ++c) {
+                    mbar_wait(&acc_empty[ab], aph ^ 1);
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem + ab * T3_ACC_COLS;
+                    const uint32_t bst = smem_base + T3_OFF_B + sb * T3_BSTAGE;
+#pragma unroll
+                    for (int ks = 0; ks < 2; ++ks) {
+                        mbar_wait(&a_ready[sa], pa);       // A slot written and (ks == 0) B chunk landed, in both CTAs
+                        tc_fence_after();
+                        const uint32_t a0 = tmem + T3_A_COL0 + sa * 32;
+                        auto bdesc = [&](uint32_t part, uint32_t slot) {
+                            return make_desc(bst + part * 128u * n + slot * 64u * n + ks * 32u * n, 16u * n, 128u, 0u);
+                        };
+                        umma2_f16_ts(d_tmem, a0 + 0, bdesc(0, 0), idesc, ks);     // Q_hi [Bc|-Bs]_hi
+                        umma2_f16_ts(d_tmem, a0 + 8, bdesc(0, 0), idesc, 1u);     // Q_lo [Bc|-Bs]_hi
+                        umma2_f16_ts(d_tmem, a0 + 0, bdesc(1, 0), idesc, 1u);     // Q_hi [Bc|-Bs]_lo
+                        umma2_f16_ts(d_tmem, a0 + 16, bdesc(0, 1), idesc, 1u);    // U_hi [Bs|Bc]_hi
+                        umma2_f16_ts(d_tmem, a0 + 24, bdesc(0, 1), idesc, 1u);    // U_lo [Bs|Bc]_hi
+                        umma2_f16_ts(d_tmem, a0 + 16, bdesc(1, 1), idesc, 1u);    // U_hi [Bs|Bc]_lo
+                        umma2_commit_mc(&a_empty[sa]);
+                        if (++sa == T3_NA) { sa = 0; pa ^= 1; }
+                    }
+                    umma2_commit_mc(&b_empty[sb]);
+                    umma2_commit_mc(&acc_full[ab]);
+                    if (++sb == T3_S) { sb = 0; pb ^= 1; }
+                    if (++ab == 2) { ab = 0; aph ^= 1; }
+                }
+        }
+        __syncwarp();
+      }
+    } else if (warp < 8) {
+        // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        const int row = threadIdx.x - 128;                          // pixel row of the tile = TMEM lane
+        const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
+        uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
+        const uint32_t ready0 = mapa_u32(smem_u32(&a_ready[0]), 0);
+        for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
+            for (int c = 0; c < n_chunks; ++c) {
+                float v[64];
+                mbar_wait(&raw_full[sr], pr);
+                t3_load_raw(smem_gen + sr * T3_RAW, row, IN_MN, v);
+                const uint32_t mask = __ldg(prm.chan_mask + c);
+                if (mask != 0xFFFFFFFFu) {                          // warp-uniform: zero the zero-weight channels
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        if (!((mask >> i) & 1u)) { v[i] = 0.f; v[32 + i] = 0.f; }
+                }
+                float m = 0.f;
+#pragma unroll
+                for (int i = 0; i < 64; ++i) m = fmaxf(m, fabsf(v[i]));
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&raw_empty[sr]);         // every lane's loads have completed (values used above)
+                if (++sr == T3_R) { sr = 0; pr ^= 1; }
+                // scale 2^(141 - e) brings the chunk's largest sample into [2^14, 2^15); e clamped so both powers are normal
+                int e = (int)(__float_as_uint(m) >> 23);
+                e = min(max(e, 15), 254);
+                const float scale = __uint_as_float((uint32_t)(268 - e) << 23);
+                scales[(seq & (T3_SCALES - 1)) * T3_M + row] = __uint_as_float((uint32_t)(e - 14) << 23);   // 2^(e - 141)
+                ++seq;
+#pragma unroll
+                for (int ks = 0; ks < 2; ++ks) {
+                    uint32_t r[32];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        t3_split(v[ks * 16 + 2 * i], v[ks * 16 + 2 * i + 1], scale, r[i], r[8 + i]);
+                        t3_split(v[32 + ks * 16 + 2 * i], v[32 + ks * 16 + 2 * i + 1], scale, r[16 + i], r[24 + i]);
+                    }
+                    mbar_wait(&a_empty[sa], pa ^ 1);
+                    tc_fence_after();
+                    tmem_st32(tmem + lane_addr + T3_A_COL0 + sa * 32, r);
+                    tmem_st_wait();
+                    if (ks == 0) {                                   // the B chunk of this CTA must have landed too
+                        mbar_wait(&b_full[sb], pb);
+                        if (++sb == T3_S) { sb = 0; pb ^= 1; }
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_remote(ready0 + sa * 8);
+                    if (++sa == T3_NA) { sa = 0; pa ^= 1; }
+                }
+            }
+        }
+    } else {
+        // ===================== epilogue (both CTAs, own TMEM lanes = own 128 pixels) =====================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
+        const int q = warp & 3;
+        const int cbase = warp >= 12 ? 128 : 0;
+        const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
+        const uint32_t empty0 = mapa_u32(smem_u32(&acc_empty[0]), 0);
+        uint32_t ab = 0, aph = 0, seq = 0;
+        float acc[128];
+        for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
+            const int tp = item / prm.n_phi_tiles, j = item - tp * prm.n_phi_tiles;
+            const long long P0 = (long long)(2 * tp + (int)rank) * T3_M + q * 32;   // first pixel of this warp
+            for (int c = 0; c < n_chunks; ++c) {
+                mbar_wait(&acc_full[ab], aph);
+                tc_fence_after();
+                const float inv = scales[(seq & (T3_SCALES - 1)) * T3_M + q * 32 + lane];   // 2^-e of this pixel's chunk
+                ++seq;
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    if (cbase + g * 32 < N2) {
+                        uint32_t r[32];
+                        tmem_ld32(tmem + lane_addr + ab * T3_ACC_COLS + cbase + g * 32, r);
+                        tmem_ld_wait();
+                        if (c == 0) {
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) acc[g * 32 + i] = __uint_as_float(r[i]) * inv;
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) acc[g * 32 + i] = fmaf(__uint_as_float(r[i]), inv, acc[g * 32 + i]);
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(empty0 + ab * 8);
+                if (++ab == 2) { ab = 0; aph ^= 1; }
+            }
+#pragma unroll
+            for (int i = 0; i < 128; ++i) acc[i] *= prm.inv_scale_b;
+            EpiTile et;
+            et.n_pix = prm.n_pix;
+            et.P0 = P0;
+            et.n_phi = prm.n_phi;
+            et.k0 = j * n + (cbase >> 1);
+            et.nv = min(n, prm.n_phi - j * n) - (cbase >> 1);
+            et.seg = 2 * j + (cbase >> 7);
+            float* sT = stage_t + (warp - 8) * (32 * 33);
+            if (prm.rec) {
+                if (!OUT_LOS) epi_tile_phi_major<true>(acc, et, lane, prm.FQ, prm.FU, prm.FA, prm.rec);
+                else epi_tile_los_major<true>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, prm.rec);
+            } else {
+                if (!OUT_LOS) epi_tile_phi_major<false>(acc, et, lane, prm.FQ, prm.FU, prm.FA, nullptr);
+                else epi_tile_los_major<false>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, nullptr);
+            }
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host side
+rmsynth_status tc3_plan_init(rmsynth_plan* p) {
+    TcGeom& g = p->tc3;
+    g.kb = T3_KC;
+    g.n_phi_tiles = (p->n_phi + T3_NMAX - 1) / T3_NMAX;
+    const int per = (p->n_phi + g.n_phi_tiles - 1) / g.n_phi_tiles;
+    g.n_tile = (per + 7) & ~7;
+    const int n_chunks = (p->n_chan + T3_KC - 1) / T3_KC;
+    g.k_pad = n_chunks * T3_KC;
+    g.ctas = 2;
+    // power-of-two scale bringing max |B| = K max(w) into [2^14, 2^15)
+    double bmax = 0.0;
+    for (int i = 0; i < p->n_chan; ++i) bmax = std::max(bmax, p->K * p->w[i]);
+    int eb;
+    std::frexp(bmax, &eb);                       // bmax = f 2^eb, f in [0.5, 1)
+    p->tc3_eb = 15 - eb;                         // bmax 2^(15 - eb) in [2^14, 2^15)
+    std::vector<uint32_t> mask(n_chunks, 0u);
+    for (int i = 0; i < p->n_chan; ++i)
+        if (p->w[i] > 0.0) mask[i / T3_KC] |= 1u << (i % T3_KC);
+    RMS_CUDA(cudaMalloc(&p->d_tc3mask, sizeof(uint32_t) * n_chunks));
+    RMS_CUDA(cudaMemcpy(p->d_tc3mask, mask.data(), sizeof(uint32_t) * n_chunks, cudaMemcpyHostToDevice));
+    const size_t halves = (size_t)g.n_phi_tiles * n_chunks * 2 * 128 * g.n_tile;
+    RMS_CUDA(cudaMalloc(&p->d_tcB3, halves * sizeof(__half)));
+    dim3 grid((g.n_tile + 63) / 64, n_chunks, g.n_phi_tiles);
+    tc3_build_b_kernel<<<grid, 64>>>(p->d_delta, p->d_kw, p->d_phi, p->n_chan, p->n_phi, g.n_tile, n_chunks,
+                                     std::ldexp(1.0, p->tc3_eb), reinterpret_cast<__half*>(p->d_tcB3));
+    RMS_LAUNCH_CHECK("tc3_build_b_kernel");
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_PHI));
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_PHI));
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_LOS));
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_LOS));
+    return RMSYNTH_OK;
+}
+
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st) {
+    Tc3Params prm;
+    prm.n_pix = n_pix;
+    prm.n_chan = p->n_chan;
+    prm.n_phi = p->n_phi;
+    prm.n = p->tc3.n_tile;
+    prm.n_phi_tiles = p->tc3.n_phi_tiles;
+    prm.n_chunks = p->tc3.k_pad / T3_KC;
+    const long long pix_tiles = (n_pix + T3_M - 1) / T3_M;
+    prm.n_items = (int)((pix_tiles + 1) / 2) * prm.n_phi_tiles;
+    prm.a3d = a3d ? 1 : 0;
+    prm.inv_scale_b = (float)std::ldexp(1.0, -p->tc3_eb);
+    prm.blob = reinterpret_cast<const __half*>(p->d_tcB3);
+    prm.chan_mask = p->d_tc3mask;
+    prm.FQ = FQ;
+    prm.FU = FU;
+    prm.FA = FA;
+    prm.rec = rec;
+    const int max_clusters = p->sm_count / 2;
+    const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
+    const int grid = 2 * clusters;
+    const CUtensorMap& mq = *static_cast<const CUtensorMap*>(map_q);
+    const CUtensorMap& mu = *static_cast<const CUtensorMap*>(map_u);
+    if (in_freq && out_phi) tc3_rmsynth_kernel<1, 0><<<grid, T3_THREADS, T3_SMEM_PHI, st>>>(mq, mu, prm);
+    else if (in_freq) tc3_rmsynth_kernel<1, 1><<<grid, T3_THREADS, T3_SMEM_LOS, st>>>(mq, mu, prm);
+    else if (out_phi) tc3_rmsynth_kernel<0, 0><<<grid, T3_THREADS, T3_SMEM_PHI, st>>>(mq, mu, prm);
+    else tc3_rmsynth_kernel<0, 1><<<grid, T3_THREADS, T3_SMEM_LOS, st>>>(mq, mu, prm);
+    RMS_LAUNCH_CHECK("tc3_rmsynth_kernel");
+    return RMSYNTH_OK;
+}
+
+}  // namespace rms

@@ -18,10 +18,10 @@ def b():
 
 
 def scheme_ids(b):
-    return {"tf32x3": b.SCHEME_TF32X3, "fp32_table": b.SCHEME_FP32_TABLE, "fp32_sincos": b.SCHEME_FP32_SINCOS}
+    return {"tf32x3": b.SCHEME_TF32X3, "f16x3": b.SCHEME_F16X3, "fp32_table": b.SCHEME_FP32_TABLE, "fp32_sincos": b.SCHEME_FP32_SINCOS}
 
 
-SCHEMES = ["tf32x3", "fp32_table", "fp32_sincos"]
+SCHEMES = ["tf32x3", "f16x3", "fp32_table", "fp32_sincos"]
 LAYOUTS = [("los", "los"), ("los", "phi"), ("freq", "los"), ("freq", "phi")]
 
 
