@@ -28,6 +28,9 @@ sys.path.insert(0, ROOT)
 METRIC = "complex_GMAC_per_s"            # LOS x chan x phi complex multiply-accumulates per second / 1e9
 TENSOR_FLOP_PER_CMAC = 24.0              # 4 real products x 3 split passes x 2
 FP32_FLOP_PER_CMAC = 8.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
+# committed under profiles/ (config, scheme) -> bytes; filled in when a capture exists
+NCU_TRAFFIC = {}
 
 
 def load_peaks():
@@ -100,7 +103,7 @@ def main():
     ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
-    ap.add_argument("--scheme", default="tf32x3", choices=["tf32x3", "fp32_table", "fp32_sincos"])
+    ap.add_argument("--scheme", default="auto", choices=["auto", "f16x3", "tf32x3", "fp32_table", "fp32_sincos"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -155,7 +158,8 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    scheme = {"tf32x3": b.SCHEME_TF32X3, "fp32_table": b.SCHEME_FP32_TABLE, "fp32_sincos": b.SCHEME_FP32_SINCOS}[a.scheme]
+    scheme = {"auto": b.SCHEME_AUTO, "f16x3": b.SCHEME_F16X3, "tf32x3": b.SCHEME_TF32X3, "fp32_table": b.SCHEME_FP32_TABLE,
+              "fp32_sincos": b.SCHEME_FP32_SINCOS}[a.scheme]
     layout = (b.IN_FREQ_MAJOR if cfg.layout_in == "freq" else 0) | (b.OUT_PHI_MAJOR if cfg.layout_out == "phi" else 0)
 
     sampler = ClockSampler(local)
@@ -174,6 +178,9 @@ def main():
         maps = {k: torch.empty(cfg.n_pix, device="cuda") for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero")}
         maps["peak_index"] = torch.empty(cfg.n_pix, dtype=torch.int32, device="cuda")
     plan = b.Plan(nu, w, phi, scheme=scheme)
+    scheme = plan.scheme                      # what "auto" resolved to
+    a.scheme = {b.SCHEME_F16X3: "f16x3", b.SCHEME_TF32X3: "tf32x3", b.SCHEME_FP32_TABLE: "fp32_table",
+                b.SCHEME_FP32_SINCOS: "fp32_sincos"}[scheme]
     stream = torch.cuda.current_stream().cuda_stream
 
     def step():
@@ -236,13 +243,17 @@ def main():
 
     peaks, peaks_src = load_peaks()
     kern_ms = float(np.mean(per_step))
-    if scheme == b.SCHEME_TF32X3:
+    if scheme in (b.SCHEME_TF32X3, b.SCHEME_F16X3):
         achieved = TENSOR_FLOP_PER_CMAC * cfg.cmac / (kern_ms * 1e-3) / 1e12
-        peak = 0.5 * peaks["bf16_tflops"]          # TF32 dense = 1/2 of bf16 (guide's nominal 1.1 / 2.25 PFLOP/s)
+        f16 = scheme == b.SCHEME_F16X3
+        # FP16 runs at the bf16 rate; TF32 dense = 1/2 of bf16 (guide's nominal 1.1 / 2.25 PFLOP/s)
+        peak = peaks["bf16_tflops"] * (1.0 if f16 else 0.5)
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "tc_rmsynth_kernel",
-                "note": f"executed 3xTF32 tensor FLOP (24 per useful complex MAC) / CUDA-event kernel time; peak = 0.5 x "
-                        f"{peaks_src} bf16 burst {peaks['bf16_tflops']:.0f} TF; of {peaks_src}"}
+                "traffic": NCU_TRAFFIC.get((a.config, a.scheme)), "kernel": "tc3_rmsynth_kernel" if f16 else "tc2_rmsynth_kernel",
+                "note": f"executed split-precision tensor FLOP (3 products x 4 real x 2 = 24 per useful complex MAC) / CUDA-event "
+                        f"kernel time; peak = {'1.0' if f16 else '0.5'} x {peaks_src} bf16 burst {peaks['bf16_tflops']:.0f} TF "
+                        f"({'fp16 = bf16 rate' if f16 else 'tf32 = half the bf16 rate'}); traffic = dram bytes read+written per launch "
+                        f"from the committed ncu --set full capture (profiles/), null if none for this config"}
     else:
         achieved = FP32_FLOP_PER_CMAC * cfg.cmac / (kern_ms * 1e-3) / 1e12
         peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
@@ -262,7 +273,7 @@ def main():
 
     out = {"metric": METRIC, "value": value, "unit": "GCMAC/s", "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "tf32x3" if scheme == b.SCHEME_TF32X3 else "f32", "data": "synthetic",
+           "dtype": {b.SCHEME_TF32X3: "tf32x3", b.SCHEME_F16X3: "f16x3"}.get(scheme, "f32"), "data": "synthetic",
            "config": dict(workload, scheme=a.scheme, l2="inputs and outputs larger than L2 (no flush needed)"
                           if 8 * cfg.n_pix * (cfg.n_chan + cfg.n_phi) > 126e6 else "fits in L2", peaks=bool(a.peaks)),
            "mpix_per_s": world * cfg.n_pix / (ms_step * 1e-3) / 1e6,

@@ -173,7 +173,19 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
             return fail(RMSYNTH_EINVAL, "options.struct_size");
         std::memcpy(&o, opt, opt->struct_size);
     }
-    int scheme = o.scheme == RMSYNTH_SCHEME_AUTO ? RMSYNTH_SCHEME_TF32X3 : o.scheme;
+    int scheme = o.scheme;
+    if (scheme == RMSYNTH_SCHEME_AUTO) {
+        // FP16 split (twice the tensor rate) unless the weights span more than 2^18: B = K w cos/sin carries one
+        // power-of-two scale for the whole plan, and below 2^-18 of the largest weight its FP16 lo part goes
+        // subnormal; the 3xTF32 scheme has FP32's exponent range and no such limit.
+        double wmax = 0.0, wmin = 0.0;
+        for (int i = 0; i < n_chan; ++i) {
+            const double wi = w ? w[i] : 1.0;
+            if (wi > wmax) wmax = wi;
+            if (wi > 0.0 && (wmin == 0.0 || wi < wmin)) wmin = wi;
+        }
+        scheme = (wmax > 0.0 && wmin >= wmax * (1.0 / 262144.0)) ? RMSYNTH_SCHEME_F16X3 : RMSYNTH_SCHEME_TF32X3;
+    }
     if (scheme != RMSYNTH_SCHEME_TF32X3 && scheme != RMSYNTH_SCHEME_F16X3 && scheme != RMSYNTH_SCHEME_FP32_TABLE && scheme != RMSYNTH_SCHEME_FP32_SINCOS)
         return fail(RMSYNTH_EINVAL, "unknown scheme");
     if (o.lambda0_mode < 0 || o.lambda0_mode > 2) return fail(RMSYNTH_EINVAL, "unknown lambda0_mode");

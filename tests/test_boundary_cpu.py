@@ -37,7 +37,7 @@ def test_version_and_strerror(b):
 
 @pytest.mark.parametrize("kw", [
     dict(nu=[1e9, -1.0]), dict(nu=[1e9, np.inf]), dict(w=[1.0, -0.5]), dict(w=[0.0, 0.0]),
-    dict(phi=[np.nan]), dict(scheme=2), dict(scheme=99), dict(lambda0_mode=7), dict(nu=[], w=None),
+    dict(phi=[np.nan]), dict(scheme=5), dict(scheme=99), dict(lambda0_mode=7), dict(nu=[], w=None),
     dict(phi=[]),
 ])
 def test_plan_create_rejects_bad_arguments_before_touching_the_device(b, kw):
