@@ -103,7 +103,8 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
     float* stage_t = reinterpret_cast<float*>(smem_gen + (size_t)S * T2_STAGE + 1024);   // LOS-major transpose buffers
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // warp index through a shuffle: provably warp-uniform, so role branches are uniform and MMA operands stay in uniform registers
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
     const int n = prm.n, N2 = 2 * prm.n;
@@ -163,7 +164,9 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         __syncwarp();
       } else if (warp == 1) {
         // ===================== MMA issuer (leader CTA only) =====================
-        if (lane == 0 && rank == 0) {
+        if (rank == 0) {
+            uint32_t lead;                                       // one elected lane issues; the whole warp runs the loop
+            asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(lead));
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)IN_MN << 15) |
                                    ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
             uint32_t st = 0, ph = 0, ab = 0, aph = 0;
@@ -191,20 +194,24 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                             return IN_MN ? make_desc(a, T2_KS * 128, 512, 1u) : make_desc(a, 16, 8 * T2_ROW, 6u);
                         };
                         auto bdesc = [&](uint32_t b) { return make_desc(b, 16, 8 * T2_ROW, 6u); };
-                        umma2_tf32(d_tmem, adesc(aQ), bdesc(bh), idesc, first ^ 1u);    // Q_hi [Bc|-Bs]_hi
+                        if (lead) {
+                            umma2_tf32(d_tmem, adesc(aQ), bdesc(bh), idesc, first ^ 1u);    // Q_hi [Bc|-Bs]_hi
+                            umma2_tf32(d_tmem, adesc(aQl), bdesc(bh), idesc, 1u);           // Q_lo [Bc|-Bs]_hi
+                            umma2_tf32(d_tmem, adesc(aQ), bdesc(bl), idesc, 1u);            // Q_hi [Bc|-Bs]_lo
+                            umma2_tf32(d_tmem, adesc(aU), bdesc(bh + s1), idesc, 1u);       // U_hi [Bs|Bc]_hi
+                            umma2_tf32(d_tmem, adesc(aUl), bdesc(bh + s1), idesc, 1u);      // U_lo [Bs|Bc]_hi
+                            umma2_tf32(d_tmem, adesc(aU), bdesc(bl + s1), idesc, 1u);       // U_hi [Bs|Bc]_lo
+                            umma2_commit_mc(&empty[st]);
+                        }
+                        __syncwarp();
                         first = 0;
-                        umma2_tf32(d_tmem, adesc(aQl), bdesc(bh), idesc, 1u);           // Q_lo [Bc|-Bs]_hi
-                        umma2_tf32(d_tmem, adesc(aQ), bdesc(bl), idesc, 1u);            // Q_hi [Bc|-Bs]_lo
-                        umma2_tf32(d_tmem, adesc(aU), bdesc(bh + s1), idesc, 1u);       // U_hi [Bs|Bc]_hi
-                        umma2_tf32(d_tmem, adesc(aUl), bdesc(bh + s1), idesc, 1u);      // U_lo [Bs|Bc]_hi
-                        umma2_tf32(d_tmem, adesc(aU), bdesc(bl + s1), idesc, 1u);       // U_hi [Bs|Bc]_lo
-                        umma2_commit_mc(&empty[st]);
                         if (++st == S) { st = 0; ph ^= 1; }
                     }
-                    umma2_commit_mc(&acc_full[ab]);
+                    if (lead) umma2_commit_mc(&acc_full[ab]);
+                    __syncwarp();
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
-            if (prof) {
+            if (prof && lead) {
                 prm.prof[cluster_id * 8 + 0] = 0; prm.prof[cluster_id * 8 + 1] = w_ready;
                 prm.prof[cluster_id * 8 + 2] = w_acc; prm.prof[cluster_id * 8 + 3] = clock64() - t_begin;
             }

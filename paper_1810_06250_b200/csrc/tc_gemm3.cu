@@ -56,6 +56,22 @@ __device__ __forceinline__ void umma2_f16_ts(uint32_t d_tmem, uint32_t a_tmem, u
         "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}" ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc),
         "r"(acc) : "memory");
 }
+// Warp-uniform forms: every lane of the issuing warp executes the instruction with identical operands and `lead`
+// selects the one lane that really issues.  The operands then live in uniform registers; issuing from inside an
+// `if (lane == 0)` region instead makes the compiler wrap every MMA in an ELECT / R2UR "waterfall" (~15 instructions).
+__device__ __forceinline__ void umma2_f16_ts_u(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc,
+                                               uint32_t lead) {
+    asm volatile(
+        "{\n.reg .pred p, q;\nsetp.ne.b32 p, %4, 0;\nsetp.ne.b32 q, %5, 0;\n"
+        "@q tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}" ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc),
+        "r"(acc), "r"(lead) : "memory");
+}
+__device__ __forceinline__ void umma2_commit_mc_u(uint64_t* bar, uint32_t lead) {
+    asm volatile(
+        "{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n"
+        "@q tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n}" ::"r"(smem_u32(bar)),
+        "h"((uint16_t)3), "r"(lead) : "memory");
+}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
@@ -165,7 +181,8 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
     float* stage_t = reinterpret_cast<float*>(smem_gen + T3_OFF_STAGE_T);         // LOS-major transpose buffers
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // warp index through a shuffle: provably warp-uniform, so role branches are uniform and MMA operands stay in uniform registers
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
     const int n = prm.n, N2 = 2 * prm.n;
@@ -238,37 +255,44 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
         __syncwarp();
       } else if (warp == 1) {
-        // ===================== MMA issuer (leader CTA only) =====================
-        if (lane == 0 && rank == 0) {
-            // kind::f16: D = F32 (bit 4), A = B = F16 (0), K-major, N = 2n, M = 256
+        // ===================== MMA issuer (leader CTA only; the whole warp runs the loop, lane 0 issues) =====================
+        if (rank == 0) {
+            // kind::f16: D = F32 (bit 4), A = B = F16 (0), K-major, N = 2n, M = 256.  One B descriptor per (stage, K step);
+            // the other three differ by constants in the 16-byte address field.
+            uint32_t lead;                                       // one elected lane (elect.sync keeps the branch "uniform + 1 lane")
+            asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(lead));
+            const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0), smem_u = __shfl_sync(0xffffffffu, smem_base, 0);   // provably warp-uniform
             const uint32_t idesc = (1u << 4) | ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
-            uint32_t sa = 0, pa = 0, sb = 0, pb = 0, ab = 0, aph = 0;
+            const uint64_t dhi = make_desc(0u, 16u * n, 128u, 0u);
+            const uint32_t o_part = (128u * n) >> 4, o_slot = (64u * n) >> 4, o_ks = (32u * n) >> 4;
+            uint32_t sa = 0, pa = 0, sb = 0, ab = 0, aph = 0;
             for (int item = cluster_id; item < prm.n_items; item += n_clusters)
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&acc_empty[ab], aph ^ 1);
                     tc_fence_after();
-                    const uint32_t d_tmem = tmem + ab * T3_ACC_COLS;
-                    const uint32_t bst = smem_base + T3_OFF_B + sb * T3_BSTAGE;
+                    const uint32_t d_tmem = tmem_u + ab * T3_ACC_COLS;
+                    const uint32_t baddr = (smem_u + T3_OFF_B + sb * T3_BSTAGE) >> 4;
 #pragma unroll
                     for (int ks = 0; ks < 2; ++ks) {
                         mbar_wait(&a_ready[sa], pa);       // A slot written and (ks == 0) B chunk landed, in both CTAs
                         tc_fence_after();
-                        const uint32_t a0 = tmem + T3_A_COL0 + sa * 32;
-                        auto bdesc = [&](uint32_t part, uint32_t slot) {
-                            return make_desc(bst + part * 128u * n + slot * 64u * n + ks * 32u * n, 16u * n, 128u, 0u);
-                        };
-                        umma2_f16_ts(d_tmem, a0 + 0, bdesc(0, 0), idesc, ks);     // Q_hi [Bc|-Bs]_hi
-                        umma2_f16_ts(d_tmem, a0 + 8, bdesc(0, 0), idesc, 1u);     // Q_lo [Bc|-Bs]_hi
-                        umma2_f16_ts(d_tmem, a0 + 0, bdesc(1, 0), idesc, 1u);     // Q_hi [Bc|-Bs]_lo
-                        umma2_f16_ts(d_tmem, a0 + 16, bdesc(0, 1), idesc, 1u);    // U_hi [Bs|Bc]_hi
-                        umma2_f16_ts(d_tmem, a0 + 24, bdesc(0, 1), idesc, 1u);    // U_lo [Bs|Bc]_hi
-                        umma2_f16_ts(d_tmem, a0 + 16, bdesc(1, 1), idesc, 1u);    // U_hi [Bs|Bc]_lo
-                        umma2_commit_mc(&a_empty[sa]);
+                        const uint32_t a0 = tmem_u + T3_A_COL0 + sa * 32;
+                        const uint64_t d0 = dhi | (uint64_t)(baddr + ks * o_ks);             // hi part, slot 0
+                        if (lead) {
+                            umma2_f16_ts(d_tmem, a0 + 0, d0, idesc, ks);                      // Q_hi [Bc|-Bs]_hi
+                            umma2_f16_ts(d_tmem, a0 + 8, d0, idesc, 1u);                      // Q_lo [Bc|-Bs]_hi
+                            umma2_f16_ts(d_tmem, a0 + 0, d0 + o_part, idesc, 1u);             // Q_hi [Bc|-Bs]_lo
+                            umma2_f16_ts(d_tmem, a0 + 16, d0 + o_slot, idesc, 1u);            // U_hi [Bs|Bc]_hi
+                            umma2_f16_ts(d_tmem, a0 + 24, d0 + o_slot, idesc, 1u);            // U_lo [Bs|Bc]_hi
+                            umma2_f16_ts(d_tmem, a0 + 16, d0 + o_part + o_slot, idesc, 1u);   // U_hi [Bs|Bc]_lo
+                            umma2_commit_mc(&a_empty[sa]);
+                        }
+                        __syncwarp();
                         if (++sa == T3_NA) { sa = 0; pa ^= 1; }
                     }
-                    umma2_commit_mc(&b_empty[sb]);
-                    umma2_commit_mc(&acc_full[ab]);
-                    if (++sb == T3_S) { sb = 0; pb ^= 1; }
+                    if (lead) { umma2_commit_mc(&b_empty[sb]); umma2_commit_mc(&acc_full[ab]); }
+                    __syncwarp();
+                    if (++sb == T3_S) sb = 0;
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
         }
