@@ -107,7 +107,7 @@ class Plan:
         self.K, self.lambda0_sq, self.n_chan, self.n_phi, self.scheme = K.value, l0.value, nc.value, npz.value, sc.value
 
     def destroy(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and _lib is not None:      # _lib is None while the interpreter shuts down
             _lib.rmsynth_plan_destroy(self._h)
             self._h = None
 

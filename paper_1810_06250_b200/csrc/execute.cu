@@ -1,6 +1,7 @@
 // rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_ex / rmsynth_execute_host: argument checks,
 // scheme dispatch (rows a4-a9) and the host-streaming loop (the paper's "each datum crosses the bus
 // once" rule, with pixel chunks instead of LOS batches sized from GPU memory P:L210).
+#include <cstdlib>
 #include <cstring>
 #include "common.cuh"
 
@@ -97,7 +98,8 @@ rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, co
     const int nc = p->n_chan, np = p->n_phi;
     const bool in_freq = layout & RMSYNTH_IN_FREQ_MAJOR, out_phi = layout & RMSYNTH_OUT_PHI_MAJOR;
     // ~256 MB of device buffers per slot, two slots in flight
-    long long chunk = (256LL << 20) / (8LL * (nc + np));
+    static const long long chunk_mb = getenv("RMSYNTH_HOST_CHUNK_MB") ? atoll(getenv("RMSYNTH_HOST_CHUNK_MB")) : 256;
+    long long chunk = ((chunk_mb > 0 ? chunk_mb : 256) << 20) / (8LL * (nc + np));
     chunk = chunk / 1024 * 1024;
     if (chunk < 1024) chunk = 1024;
     if (chunk > n_pix) chunk = n_pix;
