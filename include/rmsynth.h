@@ -51,8 +51,8 @@ enum {
 
 /* Arithmetic scheme of the contraction (rows a5/a9 of the scope table).              */
 enum {
-    RMSYNTH_SCHEME_AUTO = 0,        /* F16X3, or TF32X3 when the positive weights span   */
-                                    /* more than 2^18 (see rmsynth_plan_info for the choice) */
+    RMSYNTH_SCHEME_AUTO = 0,        /* F16X3; TF32X3 when the positive weights span more */
+                                    /* than 2^18 or n_chan < 384 (rmsynth_plan_info tells) */
     RMSYNTH_SCHEME_TF32X3 = 1,      /* tcgen05 tensor cores, split-precision 3xTF32,     */
                                     /* FP32 accumulate in TMEM                           */
     RMSYNTH_SCHEME_F16X3 = 2,       /* tcgen05 tensor cores, block-scaled FP16 hi/lo split    */

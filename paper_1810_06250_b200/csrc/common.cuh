@@ -84,7 +84,7 @@ struct rmsynth_plan {
 namespace rms {
 
 rmsynth_status ensure_scratch(const rmsynth_plan* p, int slot, size_t bytes, float** out);
-enum { SCR_PEAK_REC = 0, SCR_CUBE_Q = 1, SCR_CUBE_U = 2, SCR_REPACK_Q = 3, SCR_REPACK_U = 4 };
+enum { SCR_PEAK_REC = 0, SCR_CUBE_Q = 1, SCR_CUBE_U = 2, SCR_REPACK_Q = 3, SCR_REPACK_U = 4, SCR_TILE_SYNC = 5 };
 rmsynth_status stream_scratch(const rmsynth_plan* p, cudaStream_t st, int tag, size_t bytes, float** out);
 
 // fp32_kernels.cu
@@ -109,11 +109,13 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
 // tc_gemm3.cu
 rmsynth_status tc3_plan_init(rmsynth_plan* p);
 rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st);
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
+                          cudaStream_t st);
 
 // tc_gemm2.cu
 rmsynth_status tc2_plan_init(rmsynth_plan* p);
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st);
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
+                          cudaStream_t st);
 
 }  // namespace rms

@@ -175,16 +175,18 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
     }
     int scheme = o.scheme;
     if (scheme == RMSYNTH_SCHEME_AUTO) {
-        // FP16 split (twice the tensor rate) unless the weights span more than 2^18: B = K w cos/sin carries one
+        // FP16 split (twice the tensor rate) unless (a) the weights span more than 2^18: B = K w cos/sin carries one
         // power-of-two scale for the whole plan, and below 2^-18 of the largest weight its FP16 lo part goes
-        // subnormal; the 3xTF32 scheme has FP32's exponent range and no such limit.
+        // subnormal (3xTF32 has FP32's exponent range and no such limit); or (b) there are fewer than 384 channels:
+        // the FP16 kernel's gain comes from the K loop while its per-tile costs (drains, stores) do not shrink --
+        // measured on B200 it is 1.4x faster at 800-1000 channels and 1.14x at 400.
         double wmax = 0.0, wmin = 0.0;
         for (int i = 0; i < n_chan; ++i) {
             const double wi = w ? w[i] : 1.0;
             if (wi > wmax) wmax = wi;
             if (wi > 0.0 && (wmin == 0.0 || wi < wmin)) wmin = wi;
         }
-        scheme = (wmax > 0.0 && wmin >= wmax * (1.0 / 262144.0)) ? RMSYNTH_SCHEME_F16X3 : RMSYNTH_SCHEME_TF32X3;
+        scheme = (n_chan >= 384 && wmax > 0.0 && wmin >= wmax * (1.0 / 262144.0)) ? RMSYNTH_SCHEME_F16X3 : RMSYNTH_SCHEME_TF32X3;
     }
     if (scheme != RMSYNTH_SCHEME_TF32X3 && scheme != RMSYNTH_SCHEME_F16X3 && scheme != RMSYNTH_SCHEME_FP32_TABLE && scheme != RMSYNTH_SCHEME_FP32_SINCOS)
         return fail(RMSYNTH_EINVAL, "unknown scheme");

@@ -24,19 +24,28 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+// L2 eviction policies.  The operands (Q/U tiles re-read by every depth tile of a pixel tile, and the phase-matrix
+// blobs) are loaded evict_last; the output cubes are a write-once stream and are stored evict_first, so that
+// the 8 B x N_pix x N_phi going out do not push the inputs out of L2 between two depth tiles.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
 }
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
 }
-__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
     asm volatile(
@@ -64,8 +73,9 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* r) {
           "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
         : "r"(taddr));
 }
-__device__ __forceinline__ void st_global_pred(unsigned long long addr, float v, bool pred) {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %2, 0;\n@p st.global.f32 [%0], %1;\n}" ::"l"(addr), "f"(v), "r"((int)pred) : "memory");
+__device__ __forceinline__ void st_global_pred(unsigned long long addr, float v, bool pred, uint64_t pol) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %2, 0;\n@p st.global.L2::cache_hint.f32 [%0], %1, %3;\n}" ::"l"(addr), "f"(v),
+                 "r"((int)pred), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -89,6 +99,54 @@ __device__ __forceinline__ float rn_tf32(float x) {   // round-to-nearest(-even)
     return __uint_as_float(u & 0xFFFFE000u);
 }
 
+
+// Soft lock-step of the CTAs that share a pixel-tile pair (one per depth tile and CTA rank): each TMA producer checks in
+// before it starts loading the pair's Q/U tiles and waits (bounded) until all sharers have.  The work items are dealt
+// statically, and without this the sharers drift apart by more than the ~50 us an input line survives in L2 under
+// the output stream, so every depth tile re-read the tiles from HBM (measured: 3.3x the algorithmic bytes on the
+// 2048^2 cube).  A performance hint only: the spin is bounded, correctness never depends on it.
+__device__ __forceinline__ void tile_checkin(int* counter, int expected) {
+    if (!counter) return;
+    atomicAdd(counter, 1);
+    for (int tries = 0; tries < 256; ++tries) {
+        int v;
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+        if (v >= expected) break;
+        __nanosleep(200);
+    }
+}
+
+// Static "gang" schedule of the (pixel-tile pair, depth tile) work items over the CTA pairs of the grid.
+// T = depth tiles per pixel-tile pair.  The first S = floor(n_clusters / T) T clusters work in gangs of T: a gang
+// takes one pair and its T members take one depth tile each, at the same time, so the pair's Q/U tiles are fetched
+// from HBM once and hit L2 for the other T-1 members (kept together by tile_checkin).  The n_clusters - S left-over
+// clusters take whole pairs and walk their T depth tiles one after the other (the re-reads hit L2: the same
+// cluster used the tiles one item earlier).  Of every n_clusters consecutive pairs, S go to the gangs (S/T at a
+// time) and one to each left-over cluster, so both kinds finish together.  Every role of a CTA walks the same sequence.
+struct WorkIter {
+    int T, S, n_clusters, n_pairs, cid, k;
+    __device__ __forceinline__ void init(int cluster_id, int n_clusters_, int T_, int n_pairs_) {
+        T = T_; n_clusters = n_clusters_; n_pairs = n_pairs_; cid = cluster_id; k = 0;
+        S = (n_clusters / T) * T;
+    }
+    __device__ __forceinline__ bool ganged() const { return cid < S; }
+    // next work item of this cluster: pixel-tile pair tp, depth tile j; false when the cluster is done
+    __device__ __forceinline__ bool next(int& tp, int& j) {
+        int g;
+        if (cid < S) {
+            const int sg = k * (S / T) + cid / T;          // k-th gang round, gang cid / T
+            g = (sg / S) * n_clusters + sg % S;
+            j = cid % T;
+            ++k;
+        } else {
+            g = (k / T) * n_clusters + cid;
+            j = k % T;
+            ++k;
+        }
+        tp = g;
+        return g < n_pairs;
+    }
+};
 
 // ---- cluster / 2-CTA variants
 __device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }

@@ -113,6 +113,7 @@ __device__ __forceinline__ void epi_tile_phi_major(const float (&acc)[128], cons
     unsigned long long au = (unsigned long long)(FU + (long long)t.k0 * t.n_pix + p);
     unsigned long long aa = (unsigned long long)(FA + (long long)t.k0 * t.n_pix + p);
     asm volatile("" : "+l"(aq), "+l"(au), "+l"(aa));   // keep the bases in registers (no rematerialisation)
+    const uint64_t pol = l2_policy_evict_first();
     SegScan sc;
     if (WITH_SCAN) sc.init();
 #pragma unroll
@@ -121,15 +122,15 @@ __device__ __forceinline__ void epi_tile_phi_major(const float (&acc)[128], cons
             if (FQ) {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    st_global_pred(aq + (g * 8 + e) * sb, acc[g * 16 + e], in && g * 8 + e < t.nv);
-                    st_global_pred(au + (g * 8 + e) * sb, acc[g * 16 + 8 + e], in && g * 8 + e < t.nv);
+                    st_global_pred(aq + (g * 8 + e) * sb, acc[g * 16 + e], in && g * 8 + e < t.nv, pol);
+                    st_global_pred(au + (g * 8 + e) * sb, acc[g * 16 + 8 + e], in && g * 8 + e < t.nv, pol);
                 }
             }
             if (FA) {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     const float q = acc[g * 16 + e], u = acc[g * 16 + 8 + e];
-                    st_global_pred(aa + (g * 8 + e) * sb, sqrtf(fmaf(q, q, u * u)), in && g * 8 + e < t.nv);
+                    st_global_pred(aa + (g * 8 + e) * sb, sqrtf(fmaf(q, q, u * u)), in && g * 8 + e < t.nv, pol);
                 }
             }
             if (WITH_SCAN) sc.group(acc, g, t.nv);
@@ -150,6 +151,7 @@ __device__ __forceinline__ void epi_tile_los_major(const float (&acc)[128], cons
     const int e16 = lane & 15;                                    // depth within the block this lane stores
     const bool is_u = lane >= 16;
     const int src = (e16 >> 3) * 16 + (e16 & 7) + (is_u ? 8 : 0); // its column inside the 32-column block
+    const uint64_t pol = l2_policy_evict_first();
     SegScan sc;
     if (WITH_SCAN) sc.init();
 #pragma unroll
@@ -162,7 +164,7 @@ __device__ __forceinline__ void epi_tile_los_major(const float (&acc)[128], cons
                 __syncwarp();
                 unsigned long long a = (unsigned long long)((is_u ? FU : FQ) + t.P0 * t.n_phi + t.k0 + b * 16 + e16);
 #pragma unroll 8
-                for (int r = 0; r < 32; ++r) st_global_pred(a + r * rb, sT[r * 33 + src], ok && r < rows);
+                for (int r = 0; r < 32; ++r) st_global_pred(a + r * rb, sT[r * 33 + src], ok && r < rows, pol);
                 __syncwarp();
             }
             if (FA) {   // |F|: 16 depths per block -> lanes 0-15 store rows r, lanes 16-31 rows r+16
@@ -176,7 +178,7 @@ __device__ __forceinline__ void epi_tile_los_major(const float (&acc)[128], cons
 #pragma unroll 8
                 for (int r = 0; r < 16; ++r) {
                     const int rr = r + (is_u ? 16 : 0);
-                    st_global_pred(a + rr * rb, sT[rr * 33 + e16], ok && rr < rows);
+                    st_global_pred(a + rr * rb, sT[rr * 33 + e16], ok && rr < rows, pol);
                 }
                 __syncwarp();
             }

@@ -143,8 +143,17 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
         size_t bytes = sizeof(float) * 8 * (size_t)n_seg * (size_t)n_pix;
         if ((s = stream_scratch(p, st, SCR_PEAK_REC, bytes, &rec))) return s;
     }
-    s = f16 ? tc3_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, st)
-            : tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, st);
+    // check-in counters for the soft lock-step of the CTAs sharing a pixel-tile pair (tc_common.cuh: tile_checkin)
+    int* tile_sync = nullptr;
+    const long long n_pairs = ((n_pix + TC_M - 1) / TC_M + 1) / 2;
+    if ((f16 ? p->tc3.n_phi_tiles : p->tc.n_phi_tiles) > 1 && n_pairs > p->sm_count / 2) {
+        float* buf;
+        if ((s = stream_scratch(p, st, SCR_TILE_SYNC, sizeof(int) * (size_t)n_pairs, &buf))) return s;
+        tile_sync = reinterpret_cast<int*>(buf);
+        RMS_CUDA(cudaMemsetAsync(tile_sync, 0, sizeof(int) * (size_t)n_pairs, st));
+    }
+    s = f16 ? tc3_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, tile_sync, st)
+            : tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, tile_sync, st);
     if (s) return s;
     if (!want_maps) return RMSYNTH_OK;
     return peaks_combine(p, rec, n_seg, n_pix, amp, phi, pa0, paz, idx, st);

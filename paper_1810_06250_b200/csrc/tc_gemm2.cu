@@ -78,12 +78,13 @@ __global__ void tc2_build_b_kernel(const double* __restrict__ delta, const doubl
 
 struct Tc2Params {
     long long n_pix;
-    int n_chan, n_phi, n, n_phi_tiles, n_stages, n_items, a3d;
+    int n_chan, n_phi, n, n_phi_tiles, n_stages, n_items, n_pairs, a3d;
     const float* blob;
     float* FQ;           // may be NULL (maps only)
     float* FU;
     float* FA;           // |F| cube (Eq. 17), may be NULL
     float* rec;          // peak-segment records (tc_epilogue.cuh), NULL = no peak search
+    int* tile_sync;      // [pixel-tile pairs] check-in counters (tile_checkin), NULL = off
     long long* prof;
 };
 
@@ -131,10 +132,14 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       if (warp == 0) {
         // ===================== TMA producer (both CTAs) =====================
         if (lane == 0) {
+            const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
-            for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
-                const int tp = item / prm.n_phi_tiles, j = item - tp * prm.n_phi_tiles;
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j)) {
                 const int pix0 = (2 * tp + (int)rank) * T2_M;       // may lie past n_pix: TMA zero-fills
+                tile_checkin(prm.tile_sync && wi.ganged() ? prm.tile_sync + tp : nullptr, 2 * prm.n_phi_tiles);
                 const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) +
                                       ((size_t)j * prm.n_stages * 2 + rank) * 2 * b_part_bytes;
                 for (int s = 0; s < prm.n_stages; ++s) {
@@ -143,20 +148,20 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     const uint32_t sb = smem_base + st * T2_STAGE;
                     if (IN_MN) {
                         if (prm.a3d) {
-                            tma_load_3d(sb, &mapQ, 0, s * T2_KS, pix0 / 32, &full[st]);
-                            tma_load_3d(sb + T2_APART, &mapU, 0, s * T2_KS, pix0 / 32, &full[st]);
+                            tma_load_3d(sb, &mapQ, 0, s * T2_KS, pix0 / 32, &full[st], pol);
+                            tma_load_3d(sb + T2_APART, &mapU, 0, s * T2_KS, pix0 / 32, &full[st], pol);
                         } else {
 #pragma unroll
                             for (int g = 0; g < 4; ++g) {
-                                tma_load_2d(sb + g * (T2_KS * 128), &mapQ, pix0 + 32 * g, s * T2_KS, &full[st]);
-                                tma_load_2d(sb + T2_APART + g * (T2_KS * 128), &mapU, pix0 + 32 * g, s * T2_KS, &full[st]);
+                                tma_load_2d(sb + g * (T2_KS * 128), &mapQ, pix0 + 32 * g, s * T2_KS, &full[st], pol);
+                                tma_load_2d(sb + T2_APART + g * (T2_KS * 128), &mapU, pix0 + 32 * g, s * T2_KS, &full[st], pol);
                             }
                         }
                     } else {
-                        tma_load_2d(sb, &mapQ, s * T2_KS, pix0, &full[st]);
-                        tma_load_2d(sb + T2_APART, &mapU, s * T2_KS, pix0, &full[st]);
+                        tma_load_2d(sb, &mapQ, s * T2_KS, pix0, &full[st], pol);
+                        tma_load_2d(sb + T2_APART, &mapU, s * T2_KS, pix0, &full[st], pol);
                     }
-                    bulk_load(sb + 4 * T2_APART, bsrc + (size_t)s * 4 * b_part_bytes, 2 * b_part_bytes, &full[st]);
+                    bulk_load(sb + 4 * T2_APART, bsrc + (size_t)s * 4 * b_part_bytes, 2 * b_part_bytes, &full[st], pol);
                     if (++st == S) { st = 0; ph ^= 1; }
                 }
             }
@@ -172,7 +177,10 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             uint32_t st = 0, ph = 0, ab = 0, aph = 0;
             long long w_ready = 0, w_acc = 0, t_begin = clock64(), t0 = 0;
             const bool prof = prm.prof != nullptr;
-            for (int item = cluster_id; item < prm.n_items; item += n_clusters)
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j))
                 for (int c = 0; c < n_chunks; ++c) {
                     if (prof) t0 = clock64();
                     mbar_wait(&acc_empty[ab], aph ^ 1);
@@ -223,7 +231,13 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const int tt = threadIdx.x - 128;
         uint32_t st = 0, ph = 0;
-        const long long total = (long long)((prm.n_items - cluster_id + n_clusters - 1) / n_clusters) * prm.n_stages;
+        long long total = 0;                                 // stages this cluster will see = its work items x n_stages
+        {
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j)) total += prm.n_stages;
+        }
         for (long long it = 0; it < total; ++it) {
             mbar_wait(&full[st], ph);
             uint8_t* sg = smem_gen + (size_t)st * T2_STAGE;
@@ -254,8 +268,10 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         float acc[128];
         const bool prof = prm.prof != nullptr && warp == 8 && rank == 0;
         long long e_wait = 0, e_drain = 0, e_store = 0, e_scan = 0, t0 = 0, t1 = 0;
-        for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
-            const int tp = item / prm.n_phi_tiles, j = item - tp * prm.n_phi_tiles;
+        WorkIter wi;
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        int tp, j;
+        while (wi.next(tp, j)) {
             const long long P0 = (long long)(2 * tp + (int)rank) * T2_M + q * 32;   // first pixel of this warp
             for (int c = 0; c < n_chunks; ++c) {
                 if (prof) t0 = clock64();
@@ -329,7 +345,8 @@ rmsynth_status tc2_plan_init(rmsynth_plan* p) {
 }
 
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st) {
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
+                          cudaStream_t st) {
     Tc2Params prm;
     prm.n_pix = n_pix;
     prm.n_chan = p->n_chan;
@@ -338,13 +355,15 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.n_phi_tiles = p->tc.n_phi_tiles;
     prm.n_stages = p->tc.k_pad / T2_KS;
     const long long pix_tiles = (n_pix + T2_M - 1) / T2_M;
-    prm.n_items = (int)((pix_tiles + 1) / 2) * prm.n_phi_tiles;
+    prm.n_pairs = (int)((pix_tiles + 1) / 2);
+    prm.n_items = prm.n_pairs * prm.n_phi_tiles;
     prm.a3d = a3d ? 1 : 0;
     prm.blob = p->d_tcB2;
     prm.FQ = FQ;
     prm.FU = FU;
     prm.FA = FA;
     prm.rec = rec;
+    prm.tile_sync = tile_sync;
     prm.prof = nullptr;
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;

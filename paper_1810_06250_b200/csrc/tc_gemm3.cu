@@ -124,7 +124,7 @@ __global__ void tc3_build_b_kernel(const double* __restrict__ delta, const doubl
 
 struct Tc3Params {
     long long n_pix;
-    int n_chan, n_phi, n, n_phi_tiles, n_chunks, n_items, a3d;
+    int n_chan, n_phi, n, n_phi_tiles, n_chunks, n_items, n_pairs, a3d;
     float inv_scale_b;            // 2^-eB
     const __half* blob;
     const uint32_t* chan_mask;    // [n_chunks] bit i: channel 32 c + i exists and has w > 0
@@ -132,6 +132,7 @@ struct Tc3Params {
     float* FU;
     float* FA;                    // |F| cube, may be NULL
     float* rec;                   // peak-segment records, NULL = no peak search
+    int* tile_sync;               // [pixel-tile pairs] check-in counters (tile_checkin), NULL = off
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -210,28 +211,32 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       if (warp == 0) {
         // ===================== raw-tile TMA producer (both CTAs) =====================
         if (lane == 0) {
+            const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
-            for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
-                const int tp = item / prm.n_phi_tiles;
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j)) {
                 const int pix0 = (2 * tp + (int)rank) * T3_M;       // may lie past n_pix: TMA zero-fills
+                tile_checkin(prm.tile_sync && wi.ganged() ? prm.tile_sync + tp : nullptr, 2 * prm.n_phi_tiles);
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&raw_empty[st], ph ^ 1);
                     mbar_expect_tx(&raw_full[st], T3_RAW);
                     const uint32_t sb = smem_base + st * T3_RAW;
                     if (IN_MN) {
                         if (prm.a3d) {   // one box per operand: 32 pixels x 32 channels x 4 pixel groups
-                            tma_load_3d(sb, &mapQ, 0, c * T3_KC, pix0 / 32, &raw_full[st]);
-                            tma_load_3d(sb + T3_RAW / 2, &mapU, 0, c * T3_KC, pix0 / 32, &raw_full[st]);
+                            tma_load_3d(sb, &mapQ, 0, c * T3_KC, pix0 / 32, &raw_full[st], pol);
+                            tma_load_3d(sb + T3_RAW / 2, &mapU, 0, c * T3_KC, pix0 / 32, &raw_full[st], pol);
                         } else {
 #pragma unroll
                             for (int g = 0; g < 4; ++g) {
-                                tma_load_2d(sb + g * 4096, &mapQ, pix0 + 32 * g, c * T3_KC, &raw_full[st]);
-                                tma_load_2d(sb + T3_RAW / 2 + g * 4096, &mapU, pix0 + 32 * g, c * T3_KC, &raw_full[st]);
+                                tma_load_2d(sb + g * 4096, &mapQ, pix0 + 32 * g, c * T3_KC, &raw_full[st], pol);
+                                tma_load_2d(sb + T3_RAW / 2 + g * 4096, &mapU, pix0 + 32 * g, c * T3_KC, &raw_full[st], pol);
                             }
                         }
                     } else {             // [pix][chan]: one box of 32 channels x 128 pixels per operand
-                        tma_load_2d(sb, &mapQ, c * T3_KC, pix0, &raw_full[st]);
-                        tma_load_2d(sb + T3_RAW / 2, &mapU, c * T3_KC, pix0, &raw_full[st]);
+                        tma_load_2d(sb, &mapQ, c * T3_KC, pix0, &raw_full[st], pol);
+                        tma_load_2d(sb + T3_RAW / 2, &mapU, c * T3_KC, pix0, &raw_full[st], pol);
                     }
                     if (++st == T3_R) { st = 0; ph ^= 1; }
                 }
@@ -241,14 +246,17 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       } else if (warp == 2) {
         // ===================== B producer (both CTAs): one bulk copy per chunk =====================
         if (lane == 0) {
+            const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
-            for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
-                const int j = item % prm.n_phi_tiles;
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j)) {
                 const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) + ((size_t)j * n_chunks * 2 + rank) * b_bytes;
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&b_empty[st], ph ^ 1);
                     mbar_expect_tx(&b_full[st], b_bytes);
-                    bulk_load(smem_base + T3_OFF_B + st * T3_BSTAGE, bsrc + (size_t)c * 2 * b_bytes, b_bytes, &b_full[st]);
+                    bulk_load(smem_base + T3_OFF_B + st * T3_BSTAGE, bsrc + (size_t)c * 2 * b_bytes, b_bytes, &b_full[st], pol);
                     if (++st == T3_S) { st = 0; ph ^= 1; }
                 }
             }
@@ -266,7 +274,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const uint64_t dhi = make_desc(0u, 16u * n, 128u, 0u);
             const uint32_t o_part = (128u * n) >> 4, o_slot = (64u * n) >> 4, o_ks = (32u * n) >> 4;
             uint32_t sa = 0, pa = 0, sb = 0, ab = 0, aph = 0;
-            for (int item = cluster_id; item < prm.n_items; item += n_clusters)
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            int tp, j;
+            while (wi.next(tp, j))
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&acc_empty[ab], aph ^ 1);
                     tc_fence_after();
@@ -305,7 +316,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
         const uint32_t ready0 = mapa_u32(smem_u32(&a_ready[0]), 0);
-        for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
+        WorkIter wi;
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        int tp, j;
+        while (wi.next(tp, j)) {
             for (int c = 0; c < n_chunks; ++c) {
                 float v[64];
                 mbar_wait(&raw_full[sr], pr);
@@ -360,8 +374,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const uint32_t empty0 = mapa_u32(smem_u32(&acc_empty[0]), 0);
         uint32_t ab = 0, aph = 0, seq = 0;
         float acc[128];
-        for (int item = cluster_id; item < prm.n_items; item += n_clusters) {
-            const int tp = item / prm.n_phi_tiles, j = item - tp * prm.n_phi_tiles;
+        WorkIter wi;
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        int tp, j;
+        while (wi.next(tp, j)) {
             const long long P0 = (long long)(2 * tp + (int)rank) * T3_M + q * 32;   // first pixel of this warp
             for (int c = 0; c < n_chunks; ++c) {
                 mbar_wait(&acc_full[ab], aph);
@@ -448,7 +464,8 @@ rmsynth_status tc3_plan_init(rmsynth_plan* p) {
 }
 
 rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, cudaStream_t st) {
+                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
+                          cudaStream_t st) {
     Tc3Params prm;
     prm.n_pix = n_pix;
     prm.n_chan = p->n_chan;
@@ -457,7 +474,8 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.n_phi_tiles = p->tc3.n_phi_tiles;
     prm.n_chunks = p->tc3.k_pad / T3_KC;
     const long long pix_tiles = (n_pix + T3_M - 1) / T3_M;
-    prm.n_items = (int)((pix_tiles + 1) / 2) * prm.n_phi_tiles;
+    prm.n_pairs = (int)((pix_tiles + 1) / 2);
+    prm.n_items = prm.n_pairs * prm.n_phi_tiles;
     prm.a3d = a3d ? 1 : 0;
     prm.inv_scale_b = (float)std::ldexp(1.0, -p->tc3_eb);
     prm.blob = reinterpret_cast<const __half*>(p->d_tcB3);
@@ -466,6 +484,7 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.FU = FU;
     prm.FA = FA;
     prm.rec = rec;
+    prm.tile_sync = tile_sync;
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
     const int grid = 2 * clusters;

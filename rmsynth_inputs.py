@@ -105,6 +105,11 @@ CONFIGS = {
     3: _cfg(3, "mwa_1024", 1024, 768, 170e6, 231e6, -50.0, 50.0, 0.1, "uniform_half_one", "sparse_snr", 1.0, "los", "los"),
     4: _cfg(4, "ska_broadband_512", 512, 1000, 1.0e9, 2.0e9, -1000.0, 1000.0, 4.0, "unit", "two_sources", 0.02, "freq", "phi"),
     5: _cfg(5, "survey_2048", 2048, 400, 120e6, 168e6, -200.0, 200.0, 1.0, "unit", "thirty_percent", 0.05, "freq", "phi"),
+    # Shapes of the paper's own Table 1 runs as synthetic cubes: context workloads, not BASELINE
+    # configs.  WSRT: 512^2 x 803 -> 401 (band edges and phi range are my choice: the paper does not print them);
+    # LOFAR_LR: 540^2 x 856 channels 120.238-166.087 MHz -> 7000 depths.
+    6: _cfg(6, "paper_wsrt_512", 512, 803, 1.30e9, 1.76e9, -400.0, 400.0, 2.0, "unit", "two_sources", 0.02, "freq", "phi"),
+    7: _cfg(7, "paper_lofar_lr_540", 540, 856, 120.238e6, 166.087e6, -350.0, 349.9, 0.1, "unit", "one_source", 0.05, "freq", "phi"),
 }
 
 

@@ -161,6 +161,40 @@ def test_coherent_worst_case_and_dynamic_range(b, oracle_mod, scheme):
     plan.destroy()
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_flagged_channels_full_of_interference(b, oracle_mod, scheme):
+    """Reading A13: a zero-weight channel contributes nothing, whatever (finite) garbage it holds.  Samples of
+    1e30 in flagged channels next to O(1) data must neither change the result nor cost accuracy (the FP16 split
+    scales each 32-channel chunk by its largest sample over the channels with w > 0 only)."""
+    cfg, nu, w, phi, q, u = inputs(2, 300, start=11)
+    flagged = np.flatnonzero(w == 0)
+    assert flagged.size == 80
+    q, u = q.copy(), u.copy()
+    q[::3, flagged[::2]] = 1e30
+    u[1::3, flagged[1::2]] = -3e28
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    assert np.all(np.isfinite(FQ)) and np.all(T < 10)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, "freq", "phi")
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} flagged garbage")
+    out = run_gpu(b, plan, q, u, "los", "los")
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} flagged garbage los")
+    plan.destroy()
+
+
+def test_auto_scheme_choice(b):
+    """AUTO = FP16X3, except when the positive weights span more than 2^18 or there are < 384 channels (then 3xTF32)."""
+    phi = np.linspace(-10, 10, 9)
+    assert b.Plan(np.linspace(1e9, 2e9, 383), None, phi).scheme == b.SCHEME_TF32X3
+    nu = np.linspace(1e9, 2e9, 512)
+    w = np.ones(512)
+    assert b.Plan(nu, w, phi).scheme == b.SCHEME_F16X3
+    w[5] = 0.0
+    assert b.Plan(nu, w, phi).scheme == b.SCHEME_F16X3            # zero weights do not count
+    w[7] = 1e-7
+    assert b.Plan(nu, w, phi).scheme == b.SCHEME_TF32X3
+
+
 # ------------------------------------------------------------------ peak maps (row a7)
 @pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("lin,lout", [("freq", "phi"), ("los", "los")])
