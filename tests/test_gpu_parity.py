@@ -137,6 +137,51 @@ def test_odd_shapes_and_degenerate_sizes(b, oracle_mod, scheme, n_chan, n_phi, n
     plan.destroy()
 
 
+@pytest.mark.parametrize("scheme", ["tf32x3", "f16x3"])
+@pytest.mark.parametrize("n_pix,n_chan,n_phi", [(773, 40, 2100), (17925, 8, 2100), (5000, 33, 105), (128 * 2 * 75, 16, 230)])
+def test_work_schedule_shapes(b, oracle_mod, scheme, n_pix, n_chan, n_phi):
+    """The gang schedule (tc_common.cuh: WorkIter) at shapes that exercise its corners: more depth tiles than a
+    third of the CTA pairs (gangs of 17-21, left-over pairs walking depth tiles sequentially), fewer pixel-tile
+    pairs than gangs, more pairs than one round, one / two / three depth tiles.  Every output must be written
+    exactly once: the buffers are NaN-filled and compared in full with the oracle."""
+    rng = np.random.default_rng(n_pix + n_phi)
+    nu = np.linspace(1.0e9, 1.6e9, n_chan)
+    phi = np.linspace(-500.0, 500.0, n_phi)
+    q = rng.standard_normal((n_pix, n_chan)).astype(np.float32)
+    u = rng.standard_normal((n_pix, n_chan)).astype(np.float32)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, None, phi, q, u)
+    plan = b.Plan(nu, None, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, "freq" if n_pix % 2 == 0 else "los", "phi", peaks=True)
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} schedule {n_pix}x{n_chan}x{n_phi}")
+    check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], float(phi[1] - phi[0]), f"{scheme} schedule")
+    plan.destroy()
+
+
+def test_concurrent_streams_share_a_plan(b, oracle_mod):
+    """Two streams, one plan: per-call workspace (peak records, check-in counters) is keyed by stream."""
+    cfg, nu, w, phi, q, u = inputs(4, 3000)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    dq, du = torch.from_numpy(q).cuda(), torch.from_numpy(u).cuda()
+    outs = []
+    for rep in range(3):
+        for s in streams:
+            idx = torch.full((3000,), -1, dtype=torch.int32, device="cuda")
+            fq = torch.full((3000, plan.n_phi), float("nan"), device="cuda")
+            fu = torch.full_like(fq, float("nan"))
+            s.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(s):
+                plan.execute_peaks(dq, du, 3000, 0, fq, fu, peak_index=idx, stream=s.cuda_stream)
+            outs.append((fq, fu, idx))
+    torch.cuda.synchronize()
+    ref = oracle_mod.peaks(op, FQ, FU)["kstar"]
+    for fq, fu, idx in outs:
+        check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, "concurrent streams")
+        assert (idx.cpu().numpy() == ref).mean() > 0.99
+    plan.destroy()
+
+
 @pytest.mark.parametrize("scheme", SCHEMES)
 def test_coherent_worst_case_and_dynamic_range(b, oracle_mod, scheme):
     """All channels in phase at an on-grid depth (partial sums grow to the full norm: the worst
