@@ -207,7 +207,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const uint32_t tmem = *tmem_slot;
 
     if (warp < 4) {
-      asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
       if (warp == 0) {
         // ===================== raw-tile TMA producer (both CTAs) =====================
         if (lane == 0) {
@@ -311,7 +311,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       }
     } else if (warp < 8) {
         // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 112;");
         const int row = threadIdx.x - 128;                          // pixel row of the tile = TMEM lane
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
@@ -330,9 +330,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     for (int i = 0; i < 32; ++i)
                         if (!((mask >> i) & 1u)) { v[i] = 0.f; v[32 + i] = 0.f; }
                 }
-                float m = 0.f;
+                float m4[4] = {0.f, 0.f, 0.f, 0.f};                  // four independent chains, not one of 64 dependent maxima
 #pragma unroll
-                for (int i = 0; i < 64; ++i) m = fmaxf(m, fabsf(v[i]));
+                for (int i = 0; i < 64; ++i) m4[i & 3] = fmaxf(m4[i & 3], fabsf(v[i]));
+                const float m = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&raw_empty[sr]);         // every lane's loads have completed (values used above)
                 if (++sr == T3_R) { sr = 0; pr ^= 1; }
@@ -342,6 +343,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 const float scale = __uint_as_float((uint32_t)(268 - e) << 23);
                 scales[(seq & (T3_SCALES - 1)) * T3_M + row] = __uint_as_float((uint32_t)(e - 14) << 23);   // 2^(e - 141)
                 ++seq;
+                // Both 16-channel slots are written before the one tcgen05.wait::st: the second conversion overlaps the
+                // first store, and the chunk pays one store round trip instead of two.
+                const uint32_t s0 = sa, s1 = sa + 1 == T3_NA ? 0 : sa + 1;
+                const uint32_t p0 = pa, p1 = sa + 1 == T3_NA ? pa ^ 1 : pa;
 #pragma unroll
                 for (int ks = 0; ks < 2; ++ks) {
                     uint32_t r[32];
@@ -350,19 +355,19 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                         t3_split(v[ks * 16 + 2 * i], v[ks * 16 + 2 * i + 1], scale, r[i], r[8 + i]);
                         t3_split(v[32 + ks * 16 + 2 * i], v[32 + ks * 16 + 2 * i + 1], scale, r[16 + i], r[24 + i]);
                     }
-                    mbar_wait(&a_empty[sa], pa ^ 1);
+                    mbar_wait(&a_empty[ks ? s1 : s0], (ks ? p1 : p0) ^ 1);
                     tc_fence_after();
-                    tmem_st32(tmem + lane_addr + T3_A_COL0 + sa * 32, r);
-                    tmem_st_wait();
-                    if (ks == 0) {                                   // the B chunk of this CTA must have landed too
-                        mbar_wait(&b_full[sb], pb);
-                        if (++sb == T3_S) { sb = 0; pb ^= 1; }
-                    }
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_remote(ready0 + sa * 8);
-                    if (++sa == T3_NA) { sa = 0; pa ^= 1; }
+                    tmem_st32(tmem + lane_addr + T3_A_COL0 + (ks ? s1 : s0) * 32, r);
                 }
+                tmem_st_wait();
+                mbar_wait(&b_full[sb], pb);                          // the B chunk of this CTA must have landed too
+                if (++sb == T3_S) { sb = 0; pb ^= 1; }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { mbar_arrive_remote(ready0 + s0 * 8); mbar_arrive_remote(ready0 + s1 * 8); }
+                pa = p1;
+                sa = s1 + 1 == T3_NA ? 0 : s1 + 1;
+                if (sa == 0) pa ^= 1;
             }
         }
     } else {
