@@ -108,8 +108,8 @@ rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, co
         if (!p->hs[b]) RMS_CUDA(cudaStreamCreateWithFlags(&p->hs[b], cudaStreamNonBlocking));
         if ((s = ensure_scratch(p, 4 * b + 0, sizeof(float) * chunk * nc, &dQ[b])) ||
             (s = ensure_scratch(p, 4 * b + 1, sizeof(float) * chunk * nc, &dU[b])) ||
-            (s = ensure_scratch(p, 4 * b + 2, sizeof(float) * chunk * np, &dFQ[b])) ||
-            (s = ensure_scratch(p, 4 * b + 3, sizeof(float) * chunk * np, &dFU[b])) ||
+            (s = ensure_scratch(p, 4 * b + 2, FQ ? sizeof(float) * chunk * np : 0, &dFQ[b])) ||    // maps only: no cube buffers
+            (s = ensure_scratch(p, 4 * b + 3, FQ ? sizeof(float) * chunk * np : 0, &dFU[b])) ||
             (s = ensure_scratch(p, 8 + b, sizeof(float) * chunk * 5, &dM[b])))
             return s;
     }

@@ -330,6 +330,9 @@ def test_execute_host_matches_oracle(b, oracle_mod, scheme, lin, lout):
     out = run_gpu(b, plan, q, u, lin, lout, peaks=True, host=True)
     check_cubes(out["FQ"], out["FU"], FQ, FU, T, "execute_host")
     check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], cfg.dphi, "execute_host")
+    out2 = run_gpu(b, plan, q, u, lin, lout, peaks=True, cubes=False, host=True)      # maps only: no cube crosses the bus
+    for k, v in out["maps"].items():
+        assert np.array_equal(v, out2["maps"][k]), k
     plan.destroy()
 
 
