@@ -100,7 +100,8 @@ rmsynth_status rmsynth_plan_phase_matrix(const rmsynth_plan *plan, float *cos_kw
  *   stream  a cudaStream_t (NULL = default stream).  The call only enqueues work; it never
  *           synchronises and never allocates after the plan's first use on a shape.
  * n_pix == 0 is a successful no-op.  EINVAL: n_pix < 0, NULL Q/U/FQ/FU, unknown layout bits.
- * Non-finite samples propagate to the outputs of their pixel (no masking). */
+ * Non-finite samples propagate to the outputs of their pixel (no masking); the F16X3 scheme
+ * alone ignores the samples of zero-weight channels altogether, non-finite or not. */
 rmsynth_status rmsynth_execute(const rmsynth_plan *plan, const float *Q, const float *U,
                                long long n_pix, int layout, float *FQ, float *FU, void *stream);
 

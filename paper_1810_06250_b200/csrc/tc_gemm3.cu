@@ -207,7 +207,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const uint32_t tmem = *tmem_slot;
 
     if (warp < 4) {
-      asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
       if (warp == 0) {
         // ===================== raw-tile TMA producer (both CTAs) =====================
         if (lane == 0) {
@@ -311,7 +311,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       }
     } else if (warp < 8) {
         // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 112;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
         const int row = threadIdx.x - 128;                          // pixel row of the tile = TMEM lane
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
@@ -372,13 +372,16 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
     } else {
         // ===================== epilogue (both CTAs, own TMEM lanes = own 128 pixels) =====================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
         const int q = warp & 3;
-        const int cbase = warp >= 12 ? 128 : 0;
+        // Columns are split 112 / 96 (7 / 6 depth groups) between the two warps of a lane quarter, so that 64 staging
+        // registers fit next to the accumulators and a drain is two TMEM load round trips (~230 cycles each) instead of four.
+        const int half = warp >= 12 ? 1 : 0;
+        const int cbase = half ? 112 : 0;
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t empty0 = mapa_u32(smem_u32(&acc_empty[0]), 0);
         uint32_t ab = 0, aph = 0, seq = 0;
-        float acc[128];
+        float acc[128];                                             // 112 (half 0) or 96 (half 1) in use
         WorkIter wi;
         wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
         int tp, j;
@@ -389,19 +392,41 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 tc_fence_after();
                 const float inv = scales[(seq & (T3_SCALES - 1)) * T3_M + q * 32 + lane];   // 2^-e of this pixel's chunk
                 ++seq;
+                const uint32_t tbase = tmem + lane_addr + ab * T3_ACC_COLS + cbase;
+                {
+                    uint32_t r[64];
+                    tmem_ld64(tbase, r);
+                    tmem_ld_wait();
+                    if (c == 0) {
 #pragma unroll
-                for (int g = 0; g < 4; ++g) {
-                    if (cbase + g * 32 < N2) {
-                        uint32_t r[32];
-                        tmem_ld32(tmem + lane_addr + ab * T3_ACC_COLS + cbase + g * 32, r);
-                        tmem_ld_wait();
-                        if (c == 0) {
+                        for (int i = 0; i < 64; ++i) acc[i] = __uint_as_float(r[i]) * inv;
+                    } else {
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) acc[g * 32 + i] = __uint_as_float(r[i]) * inv;
-                        } else {
+                        for (int i = 0; i < 64; ++i) acc[i] = fmaf(__uint_as_float(r[i]), inv, acc[i]);
+                    }
+                }
+                if (!half) {
+                    uint32_t r[48];
+                    tmem_ld32(tbase + 64, r);
+                    tmem_ld16(tbase + 96, r + 32);
+                    tmem_ld_wait();
+                    if (c == 0) {
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) acc[g * 32 + i] = fmaf(__uint_as_float(r[i]), inv, acc[g * 32 + i]);
-                        }
+                        for (int i = 0; i < 48; ++i) acc[64 + i] = __uint_as_float(r[i]) * inv;
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 48; ++i) acc[64 + i] = fmaf(__uint_as_float(r[i]), inv, acc[64 + i]);
+                    }
+                } else {
+                    uint32_t r[32];
+                    tmem_ld32(tbase + 64, r);
+                    tmem_ld_wait();
+                    if (c == 0) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) acc[64 + i] = __uint_as_float(r[i]) * inv;
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) acc[64 + i] = fmaf(__uint_as_float(r[i]), inv, acc[64 + i]);
                     }
                 }
                 tc_fence_before();
@@ -410,14 +435,14 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 if (++ab == 2) { ab = 0; aph ^= 1; }
             }
 #pragma unroll
-            for (int i = 0; i < 128; ++i) acc[i] *= prm.inv_scale_b;
+            for (int i = 0; i < 112; ++i) acc[i] *= prm.inv_scale_b;
             EpiTile et;
             et.n_pix = prm.n_pix;
             et.P0 = P0;
             et.n_phi = prm.n_phi;
             et.k0 = j * n + (cbase >> 1);
-            et.nv = min(n, prm.n_phi - j * n) - (cbase >> 1);
-            et.seg = 2 * j + (cbase >> 7);
+            et.nv = min(min(n, prm.n_phi - j * n) - (cbase >> 1), half ? 48 : 56);
+            et.seg = 2 * j + half;
             float* sT = stage_t + (warp - 8) * (32 * 33);
             if (prm.rec) {
                 if (!OUT_LOS) epi_tile_phi_major<true>(acc, et, lane, prm.FQ, prm.FU, prm.FA, prm.rec);
