@@ -56,22 +56,6 @@ __device__ __forceinline__ void umma2_f16_ts(uint32_t d_tmem, uint32_t a_tmem, u
         "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}" ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc),
         "r"(acc) : "memory");
 }
-// Warp-uniform forms: every lane of the issuing warp executes the instruction with identical operands and `lead`
-// selects the one lane that really issues.  The operands then live in uniform registers; issuing from inside an
-// `if (lane == 0)` region instead makes the compiler wrap every MMA in an ELECT / R2UR "waterfall" (~15 instructions).
-__device__ __forceinline__ void umma2_f16_ts_u(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc,
-                                               uint32_t lead) {
-    asm volatile(
-        "{\n.reg .pred p, q;\nsetp.ne.b32 p, %4, 0;\nsetp.ne.b32 q, %5, 0;\n"
-        "@q tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}" ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc),
-        "r"(acc), "r"(lead) : "memory");
-}
-__device__ __forceinline__ void umma2_commit_mc_u(uint64_t* bar, uint32_t lead) {
-    asm volatile(
-        "{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n"
-        "@q tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n}" ::"r"(smem_u32(bar)),
-        "h"((uint16_t)3), "r"(lead) : "memory");
-}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
@@ -267,7 +251,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         if (rank == 0) {
             // kind::f16: D = F32 (bit 4), A = B = F16 (0), K-major, N = 2n, M = 256.  One B descriptor per (stage, K step);
             // the other three differ by constants in the 16-byte address field.
-            uint32_t lead;                                       // one elected lane (elect.sync keeps the branch "uniform + 1 lane")
+            // The whole warp runs the loop (warp index from a shuffle = provably uniform) and one elected lane issues: the
+            // MMA operands then stay in uniform registers and six UTCHMMA go out back to back.  Issued from inside an
+            // `if (lane == 0)` region, nvcc wraps every MMA in an ELECT / R2UR "waterfall" of ~15 instructions.
+            uint32_t lead;
             asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(lead));
             const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0), smem_u = __shfl_sync(0xffffffffu, smem_base, 0);   // provably warp-uniform
             const uint32_t idesc = (1u << 4) | ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
