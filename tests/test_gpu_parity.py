@@ -363,6 +363,37 @@ def test_api_edges(b):
         plan.destroy()
 
 
+def test_execute_is_capturable_in_a_cuda_graph(b, oracle_mod):
+    """rmsynth_execute only enqueues (kernels + one memset) once its per-stream workspace exists, so a launch-bound
+    loop over small cubes can be captured in a CUDA graph and replayed."""
+    cfg, nu, w, phi, q, u = inputs(1, 640)
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    for scheme in ("tf32x3", "f16x3"):
+        plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+        dq, du = torch.from_numpy(q).cuda(), torch.from_numpy(u).cuda()
+        fq = torch.zeros(640, plan.n_phi, device="cuda")
+        fu = torch.zeros_like(fq)
+        idx = torch.zeros(640, dtype=torch.int32, device="cuda")
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            plan.execute_peaks(dq, du, 640, 0, fq, fu, peak_index=idx, stream=s.cuda_stream)   # first use allocates the workspace
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(4):
+                plan.execute_peaks(dq, du, 640, 0, fq, fu, peak_index=idx, stream=torch.cuda.current_stream().cuda_stream)
+        fq.fill_(float("nan"))
+        fu.fill_(float("nan"))
+        idx.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, f"graph replay {scheme}")
+        assert int(idx.min()) >= 0
+        del g
+        plan.destroy()
+
+
 def test_nonfinite_samples_stay_in_their_pixel(b):
     nu, phi = np.linspace(1e9, 2e9, 40), np.linspace(-100, 100, 21)
     for scheme in SCHEMES:
