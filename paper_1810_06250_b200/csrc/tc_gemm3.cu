@@ -191,7 +191,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const uint32_t tmem = *tmem_slot;
 
     if (warp < 4) {
-      asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
       if (warp == 0) {
         // ===================== raw-tile TMA producer (both CTAs) =====================
         if (lane == 0) {
@@ -298,7 +298,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       }
     } else if (warp < 8) {
         // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
         const int row = threadIdx.x - 128;                          // pixel row of the tile = TMEM lane
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
