@@ -138,7 +138,7 @@ def test_odd_shapes_and_degenerate_sizes(b, oracle_mod, scheme, n_chan, n_phi, n
 
 
 @pytest.mark.parametrize("scheme", ["tf32x3", "f16x3"])
-@pytest.mark.parametrize("n_pix,n_chan,n_phi", [(773, 40, 2100), (17925, 8, 2100), (5000, 33, 105), (128 * 2 * 75, 16, 230)])
+@pytest.mark.parametrize("n_pix,n_chan,n_phi", [(773, 40, 2100), (17925, 8, 2100), (5000, 33, 105), (128 * 2 * 75, 16, 230), (300, 8, 8000)])
 def test_work_schedule_shapes(b, oracle_mod, scheme, n_pix, n_chan, n_phi):
     """The gang schedule (tc_common.cuh: WorkIter) at shapes that exercise its corners: more depth tiles than a
     third of the CTA pairs (gangs of 17-21, left-over pairs walking depth tiles sequentially), fewer pixel-tile
