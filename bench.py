@@ -30,10 +30,10 @@ TENSOR_FLOP_PER_CMAC = 24.0              # 4 real products x 3 split passes x 2 
 FP32_FLOP_PER_CMAC = 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
 # committed under profiles/ (config, scheme) -> bytes; filled in when a capture exists
-NCU_TRAFFIC = {(2, "f16x3"): 1.696726e9 + 1.644172e9,      # profiles/r01_ncu_full_tc3_cfg2.txt (algorithmic 3.358e9)
-               (5, "f16x3"): 13.429987e9 + 13.412325e9,    # profiles/r01_ncu_full_tc3_cfg5.txt (algorithmic 26.877e9)
-               (2, "tf32x3"): 1.940925e9 + 1.653829e9,     # profiles/r01_ncu_full_tc2_cfg2.txt
-               (5, "tf32x3"): 13.432560e9 + 13.415863e9}   # profiles/r01_ncu_full_tc2_cfg5.txt
+NCU_TRAFFIC = {(2, "f16x3"): 1.697770e9 + 1.644242e9,      # profiles/r01_ncu_full_tc3_cfg2.txt (algorithmic 3.358e9)
+               (5, "f16x3"): 13.427832e9 + 13.411358e9,    # profiles/r01_ncu_full_tc3_cfg5.txt (algorithmic 26.877e9)
+               (2, "tf32x3"): 1.942956e9 + 1.650126e9,     # profiles/r01_ncu_full_tc2_cfg2.txt
+               (5, "tf32x3"): 13.432003e9 + 13.415196e9}   # profiles/r01_ncu_full_tc2_cfg5.txt
 
 
 def load_peaks():
