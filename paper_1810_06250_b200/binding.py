@@ -11,8 +11,12 @@ import os
 
 import numpy as np
 
+from . import build as _build
+
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "librmsynth.so")
+# RMSYNTH_LIB selects another build of the same sources (the timeline debug build); default = the product library,
+# recompiled here if the sources on disk are not the ones it was built from (content hash, see build.py).
+LIB_PATH = os.environ.get("RMSYNTH_LIB") or _build.build()
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1810_06250_b200.build` (no CPU fallback exists)")
 _lib = C.CDLL(LIB_PATH)
@@ -83,6 +87,10 @@ def _d(a):
 
 def rmsynth_version() -> str:
     return _lib.rmsynth_version().decode()
+
+
+if not os.environ.get("RMSYNTH_LIB") and _build.source_hash() not in rmsynth_version():
+    raise ImportError(f"{LIB_PATH} was not built from the sources on disk ({rmsynth_version()} vs {_build.source_hash()})")
 
 
 def rmsynth_launch_count(reset: bool = False) -> int:

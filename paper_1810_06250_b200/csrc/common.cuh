@@ -95,6 +95,8 @@ rmsynth_status fp32_sincos_execute(const rmsynth_plan* p, const float* Q, const 
 // peaks.cu
 rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,
                              float* pa0, float* paz, int* idx, cudaStream_t st);
+rmsynth_status peaks_gather(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, const float* FQ, const float* FU,
+                            bool out_phi, float* amp, float* phi, float* pa0, float* paz, int* idx, cudaStream_t st);
 rmsynth_status abs_from_cubes(const float* FQ, const float* FU, long long n, float* FA, cudaStream_t st);
 rmsynth_status peaks_from_cubes(const rmsynth_plan* p, const float* FQ, const float* FU, long long n_pix,
                                 int out_layout, float* amp, float* phi, float* pa0, float* paz, int* idx,
@@ -108,14 +110,14 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
 
 // tc_gemm3.cu
 rmsynth_status tc3_plan_init(rmsynth_plan* p);
-rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
-                          cudaStream_t st);
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq, bool out_phi,
+                          int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
+                          int sync_lag, cudaStream_t st);
 
 // tc_gemm2.cu
 rmsynth_status tc2_plan_init(rmsynth_plan* p);
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
                           bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
-                          cudaStream_t st);
+                          int gang, int sync_lag, cudaStream_t st);
 
 }  // namespace rms

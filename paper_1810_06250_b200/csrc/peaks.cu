@@ -35,22 +35,25 @@ __global__ void __launch_bounds__(256) peaks_los_major_kernel(
     if (p >= n_pix) return;
     const float* fq = FQ + (size_t)p * n_phi;
     const float* fu = FU + (size_t)p * n_phi;
-    float best = -1.f;
+    float best = -1.f, nf = 0.f;
     int kb = 0x7fffffff;
     for (int k = lane; k < n_phi; k += 32) {
         float q = fq[k], u = fu[k];
         float y2 = fmaf(q, q, u * u);
+        nf = fmaf(y2, 0.f, nf);                    // sticky NaN once |F|^2 is not finite (reading A17)
         if (y2 > best) { best = y2; kb = k; }      // strict > keeps the lowest k per lane
     }
     for (int o = 16; o > 0; o >>= 1) {
         float ob = __shfl_xor_sync(0xffffffffu, best, o);
         int ok = __shfl_xor_sync(0xffffffffu, kb, o);
+        nf += __shfl_xor_sync(0xffffffffu, nf, o);
         if (ob > best || (ob == best && ok < kb)) { best = ob; kb = ok; }
     }
     if (lane != 0) return;
-    if (kb >= n_phi) kb = 0;                        // all-NaN row: report index 0
+    if (kb >= n_phi) kb = 0;                        // all-NaN row: flagged below
     PeakState s;
     s.init();
+    s.nonfinite = nf;
     s.best_k = kb;
     s.best_q = fq[kb];
     s.best_u = fu[kb];
@@ -79,6 +82,7 @@ __global__ void __launch_bounds__(256) peaks_combine_kernel(
         if (first == -1.f) continue;                       // empty segment (ragged last depth tile)
         if (need_next) { s.best_yp2 = first; need_next = false; }
         const float by2 = r[0];
+        s.nonfinite += by2 * 0.f;                          // NaN: the segment saw a non-finite |F|^2
         if (by2 > s.best_y2) {
             s.best_y2 = by2;
             s.best_k = __float_as_int(r[1 * n_pix]);
@@ -92,6 +96,47 @@ __global__ void __launch_bounds__(256) peaks_combine_kernel(
         last = r[7 * n_pix];
     }
     refine_and_store(s, n_phi, phif, lambda0_sq, p, amp, phi, pa0, paz, idx);
+}
+
+// Row a7, fused form when the cubes were written (tc_epilogue.cuh: LightScan): the segment records hold only
+// (max |F|^2, k); k* is the first segment maximum in ascending depth order (strict >), and the samples at k*, k* - 1,
+// k* + 1 are read back from the cubes the same launch sequence has just written -- the very FP32 values the epilogue
+// held in registers, so |F|^2 = fma(q, q, u u) reproduces the recorded maximum bit for bit.  One thread per pixel.
+__global__ void __launch_bounds__(256) peaks_gather_kernel(
+    const float* __restrict__ rec, int n_seg, long long n_pix, int n_phi, const float* __restrict__ FQ,
+    const float* __restrict__ FU, int out_phi, const float* __restrict__ phif, double lambda0_sq, float* amp, float* phi,
+    float* pa0, float* paz, int* idx) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pix) return;
+    PeakState s;
+    s.init();
+    for (int g = 0; g < n_seg; ++g) {
+        const float* r = rec + (long long)g * kPeakFields * n_pix + p;
+        const float by2 = r[0];
+        s.nonfinite += by2 * 0.f;
+        if (by2 > s.best_y2) { s.best_y2 = by2; s.best_k = __float_as_int(r[1 * n_pix]); }
+    }
+    const int k = s.best_k;
+    auto y2_at = [&](int kk, float& q, float& u) {
+        const size_t i = out_phi ? (size_t)kk * n_pix + p : (size_t)p * n_phi + kk;
+        q = FQ[i];
+        u = FU[i];
+        return fmaf(q, q, u * u);
+    };
+    float q, u;
+    s.best_y2 = y2_at(k, s.best_q, s.best_u);
+    if (k > 0) s.best_ym2 = y2_at(k - 1, q, u);
+    if (k < n_phi - 1) s.best_yp2 = y2_at(k + 1, q, u);
+    refine_and_store(s, n_phi, phif, lambda0_sq, p, amp, phi, pa0, paz, idx);
+}
+
+rmsynth_status peaks_gather(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, const float* FQ, const float* FU,
+                            bool out_phi, float* amp, float* phi, float* pa0, float* paz, int* idx, cudaStream_t st) {
+    if (n_pix == 0) return RMSYNTH_OK;
+    peaks_gather_kernel<<<(unsigned)((n_pix + 255) / 256), 256, 0, st>>>(rec, n_seg, n_pix, p->n_phi, FQ, FU, out_phi ? 1 : 0,
+                                                                          p->d_phif, p->lambda0_sq, amp, phi, pa0, paz, idx);
+    RMS_LAUNCH_CHECK("peaks_gather_kernel");
+    return RMSYNTH_OK;
 }
 
 rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,

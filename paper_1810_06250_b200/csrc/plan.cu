@@ -329,6 +329,10 @@ const char* rmsynth_strerror(rmsynth_status s) {
 }
 
 const char* rmsynth_last_error(void) { return t_last_error.c_str(); }
-const char* rmsynth_version(void) { return "rmsynth-b200 0.1 (sm_100a)"; }
+#ifndef RMSYNTH_SOURCE_HASH
+#define RMSYNTH_SOURCE_HASH "unknown"
+#endif
+// the hash is the SHA-256 prefix of the sources this binary was compiled from (paper_1810_06250_b200/build.py)
+const char* rmsynth_version(void) { return "rmsynth-b200 0.2 (sm_100a) src " RMSYNTH_SOURCE_HASH; }
 
 }  // extern "C"

@@ -47,15 +47,6 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
 }
-__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc),
-        "r"(acc) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
@@ -105,52 +96,99 @@ __device__ __forceinline__ float rn_tf32(float x) {   // round-to-nearest(-even)
 }
 
 
-// Soft lock-step of the CTAs that share a pixel-tile pair (one per depth tile and CTA rank): each TMA producer checks in
-// before it starts loading the pair's Q/U tiles and waits (bounded) until all sharers have.  The work items are dealt
-// statically, and without this the sharers drift apart by more than the ~50 us an input line survives in L2 under
-// the output stream, so every depth tile re-read the tiles from HBM (measured: 3.3x the algorithmic bytes on the
-// 2048^2 cube).  A performance hint only: the spin is bounded, correctness never depends on it.
-__device__ __forceinline__ void tile_checkin(int* counter, int expected) {
-    if (!counter) return;
-    atomicAdd(counter, 1);
+// Static "gang" schedule of the (pixel-tile pair, depth tile) work items over the CTA pairs of the grid.
+// T = depth tiles per pixel-tile pair, G = gang size (a divisor of T).  The first S = floor(n_clusters / G) G clusters
+// work in gangs of G: a gang takes one pair, member m = cid % G walks the depth tiles m, m + G, m + 2G, ... one after
+// the other, all members at the same time, so the pair's Q/U tiles are fetched from HBM once and hit L2 for every other
+// (member, depth tile) -- across members because gang_checkin keeps them together, within a member because it used the
+// same tiles one item earlier.  G = T is "one depth tile per member" (smallest L2 footprint: n_clusters / T pairs in
+// flight), G = 1 is "every cluster on its own" (no check-in at all, n_clusters pairs in flight).  The n_clusters - S
+// left-over clusters take whole pairs and walk all T depth tiles.  Of every n_clusters consecutive pairs, S go to the
+// gangs (S / G at a time) and one to each left-over cluster, so both kinds finish together.
+// Every role of a CTA walks the same sequence.
+struct WorkIter {
+    int T, G, S, n_clusters, n_pairs, cid, k;
+    __device__ __forceinline__ void init(int cluster_id, int n_clusters_, int T_, int n_pairs_, int G_) {
+        T = T_; G = G_; n_clusters = n_clusters_; n_pairs = n_pairs_; cid = cluster_id; k = 0;
+        S = (n_clusters / G) * G;
+    }
+    __device__ __forceinline__ bool ganged() const { return cid < S && G > 1; }
+    __device__ __forceinline__ int walk() const { return cid < S ? T / G : T; }     // depth tiles this cluster walks per pair
+    // pixel-tile pair of the r-th round of a ganged cluster
+    __device__ __forceinline__ int gang_pair(int r) const {
+        const int sg = r * (S / G) + cid / G;              // r-th gang round, gang cid / G
+        return (sg / S) * n_clusters + sg % S;
+    }
+    // next work item of this cluster: pixel-tile pair tp, depth tile j; false when the cluster is done
+    __device__ __forceinline__ bool next(int& tp, int& j) {
+        int g;
+        if (cid < S) {
+            const int w = T / G;
+            g = gang_pair(k / w);
+            j = cid % G + (k % w) * G;
+        } else {
+            g = (k / T) * n_clusters + cid;
+            j = k % T;
+        }
+        ++k;
+        tp = g;
+        return g < n_pairs;
+    }
+    __device__ __forceinline__ bool new_pair() const { return (k - 1) % walk() == 0; }   // the item next() just returned starts a pair
+};
+
+// Soft lock-step of the CTAs of a gang.  The work items are dealt statically and nothing else ties the members
+// together; left alone they drift apart until the tiles a leader pulled in from HBM have left L2 by the time the
+// laggards ask for them (measured on the 2048^2 cube without any check-in: 39.9 GB read for 13.4 GB algorithmic).
+// Every TMA producer therefore checks in on a per-pair counter before it loads a new pair's first tile, and waits
+// (bounded) until the whole gang has checked in for the pair it started `lag` rounds earlier: lag = 0 is a barrier
+// per pair; lag >= 1 only bounds the drift.  A performance hint only: the spin is bounded, correctness never depends on it.
+__device__ __forceinline__ void gang_checkin(int* counters, const WorkIter& wi, int tp, int lag, int expected) {
+    if (!counters || !wi.ganged() || !wi.new_pair()) return;
+    atomicAdd(counters + tp, 1);
+    const int r = (wi.k - 1) / wi.walk() - lag;            // wi.next() has already advanced k past this item
+    if (r < 0) return;
+    const int* c = counters + wi.gang_pair(r);
     for (int tries = 0; tries < 256; ++tries) {
         int v;
-        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
         if (v >= expected) break;
         __nanosleep(200);
     }
 }
 
-// Static "gang" schedule of the (pixel-tile pair, depth tile) work items over the CTA pairs of the grid.
-// T = depth tiles per pixel-tile pair.  The first S = floor(n_clusters / T) T clusters work in gangs of T: a gang
-// takes one pair and its T members take one depth tile each, at the same time, so the pair's Q/U tiles are fetched
-// from HBM once and hit L2 for the other T-1 members (kept together by tile_checkin).  The n_clusters - S left-over
-// clusters take whole pairs and walk their T depth tiles one after the other (the re-reads hit L2: the same
-// cluster used the tiles one item earlier).  Of every n_clusters consecutive pairs, S go to the gangs (S/T at a
-// time) and one to each left-over cluster, so both kinds finish together.  Every role of a CTA walks the same sequence.
-struct WorkIter {
-    int T, S, n_clusters, n_pairs, cid, k;
-    __device__ __forceinline__ void init(int cluster_id, int n_clusters_, int T_, int n_pairs_) {
-        T = T_; n_clusters = n_clusters_; n_pairs = n_pairs_; cid = cluster_id; k = 0;
-        S = (n_clusters / T) * T;
+// ---- per-role timeline (debug build only: python -m paper_1810_06250_b200.build --timeline) -----------------------
+// clock64 stamps / accumulated waits of the first TL_ITEMS work items of a few CTAs, one row of TL_SLOTS values per
+// (CTA, role, item); read back and tabulated by paper_1810_06250_b200/timeline.py.  In the product build every
+// method is empty and the optimiser removes the calls.
+constexpr int TL_ITEMS = 128, TL_SLOTS = 8, TL_ROLES = 5, TL_CTAS = 8;
+enum { TL_PRODUCER = 0, TL_ISSUER = 1, TL_TRANSFORM = 2, TL_EPI0 = 3, TL_EPI1 = 4 };
+struct TlRole {
+#ifdef RMSYNTH_TIMELINE
+    long long* base;
+    long long t0;
+    int item;
+    __device__ __forceinline__ void init(long long* buf, int role) {
+        const int b = blockIdx.x, g = gridDim.x;           // cluster 0, cluster 1, cluster 3 (same gang) and the last cluster
+        const int slot = b < 4 ? b : (b == 6 || b == 7) ? b - 2 : (g >= 10 && b >= g - 2) ? 6 + b - (g - 2) : -1;
+        base = (buf && slot >= 0 && (threadIdx.x & 31) == 0) ? buf + (size_t)(slot * TL_ROLES + role) * TL_ITEMS * TL_SLOTS : nullptr;
+        item = 0;
+        t0 = 0;
     }
-    __device__ __forceinline__ bool ganged() const { return cid < S; }
-    // next work item of this cluster: pixel-tile pair tp, depth tile j; false when the cluster is done
-    __device__ __forceinline__ bool next(int& tp, int& j) {
-        int g;
-        if (cid < S) {
-            const int sg = k * (S / T) + cid / T;          // k-th gang round, gang cid / T
-            g = (sg / S) * n_clusters + sg % S;
-            j = cid % T;
-            ++k;
-        } else {
-            g = (k / T) * n_clusters + cid;
-            j = k % T;
-            ++k;
-        }
-        tp = g;
-        return g < n_pairs;
-    }
+    __device__ __forceinline__ bool on() const { return base && item < TL_ITEMS; }
+    __device__ __forceinline__ void stamp(int s) { if (on()) base[item * TL_SLOTS + s] = clock64(); }
+    __device__ __forceinline__ void begin() { if (on()) t0 = clock64(); }
+    __device__ __forceinline__ void add(int s) { if (on()) base[item * TL_SLOTS + s] += clock64() - t0; }
+    __device__ __forceinline__ void lap(int s) { if (on()) { const long long t = clock64(); base[item * TL_SLOTS + s] += t - t0; t0 = t; } }
+    __device__ __forceinline__ void next() { ++item; }
+#else
+    __device__ __forceinline__ void init(long long*, int) {}
+    __device__ __forceinline__ void stamp(int) {}
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ void add(int) {}
+    __device__ __forceinline__ void lap(int) {}
+    __device__ __forceinline__ void next() {}
+#endif
 };
 
 // ---- cluster / 2-CTA variants
@@ -161,19 +199,10 @@ __device__ __forceinline__ void cluster_sync_all() {
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, uint32_t rank) {
     uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
 }
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {   // release at cluster scope
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
 // Remote arrival with the default (.release.cta) semantics -- the form NVIDIA's own 2-SM kernels use to signal
-// the leader CTA's barrier.  The cluster-scope release above costs ~1000 cycles per arrival (measured).
+// the leader CTA's barrier.  A cluster-scope release (.release.cluster) costs ~1000 cycles per arrival (measured).
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {   // acquire at cluster scope
-    asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\n"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 __device__ __forceinline__ void umma2_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
     asm volatile(

@@ -32,12 +32,13 @@ struct EpiTile {
 // index on ties, neighbours of the best sample tracked).  A warp's 64 depths are scanned as two independent
 // chains (depth groups 0-3 and 4-7) so that consecutive steps are not one long dependency chain.
 struct ScanChain {
-    float best, ym2, yp2, q, u, prev, first;
+    float best, ym2, yp2, q, u, prev, first, nf;
     int k;          // local depth index of the best sample
     bool wn;        // the next sample is the right-hand neighbour of the best
-    __device__ __forceinline__ void init() { best = ym2 = yp2 = prev = first = -1.f; q = u = 0.f; k = 0; wn = false; }
+    __device__ __forceinline__ void init() { best = ym2 = yp2 = prev = first = -1.f; q = u = nf = 0.f; k = 0; wn = false; }
     __device__ __forceinline__ void step(int kl, float qq, float uu) {
         const float y2 = fmaf(qq, qq, uu * uu);
+        nf = fmaf(y2, 0.f, nf);              // sticky NaN once |F|^2 is not finite (reading A17)
         yp2 = wn ? y2 : yp2;
         const bool gt = y2 > best;
         best = gt ? y2 : best;
@@ -86,7 +87,7 @@ struct SegScan {
         const long long p = t.P0 + lane;
         if (p >= t.n_pix) return;
         float* r = rec + (long long)t.seg * kPeakFields * t.n_pix + p;
-        r[0 * t.n_pix] = a.best;
+        r[0 * t.n_pix] = a.best + (a.nf + b.nf);     // NaN marks a segment that saw a non-finite |F|^2
         r[1 * t.n_pix] = __int_as_float(t.k0 + a.k);
         r[2 * t.n_pix] = a.q;
         r[3 * t.n_pix] = a.u;
@@ -186,6 +187,189 @@ __device__ __forceinline__ void epi_tile_los_major(const float (&acc)[128], cons
         }
     }
     if (WITH_SCAN) sc.finish(t, lane, rec);
+}
+
+// ---- light peak search + TMA tile stores: the tile end of the FP16 kernel when cubes are written ----------------
+// When the cubes go to memory anyway, the peak search only has to find (max |F|^2, k) per segment: the values at
+// k*, k* - 1, k* + 1 are read back from the cubes by peaks_gather_kernel (peaks.cu), 24 bytes per pixel, instead of
+// being tracked through eight selects per depth.  A group of eight depths costs 8 FFMA (|F|^2), 8 FFMA (non-finite
+// flag) and a 7-match tournament (strict >, the left = lower depth wins ties), i.e. ~5 instructions per depth.
+struct LightScan {
+    float best, nf;
+    int k;
+    __device__ __forceinline__ void init() { best = -1.f; nf = 0.f; k = 0; }
+    __device__ __forceinline__ void group(const float (&acc)[128], int g, int nv) {
+        float y[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const float q = acc[g * 16 + e], u = acc[g * 16 + 8 + e];
+            const float v = fmaf(q, q, u * u);
+            const bool ok = g * 8 + e < nv;                  // all true except in the cube's last, ragged group
+            y[e] = ok ? v : -2.f;
+            nf = fmaf(ok ? v : 0.f, 0.f, nf);
+        }
+        int i01 = y[1] > y[0], i23 = y[3] > y[2], i45 = y[5] > y[4], i67 = y[7] > y[6];
+        const float m01 = i01 ? y[1] : y[0], m23 = i23 ? y[3] : y[2], m45 = i45 ? y[5] : y[4], m67 = i67 ? y[7] : y[6];
+        const bool r03 = m23 > m01, r47 = m67 > m45;
+        const float m03 = r03 ? m23 : m01, m47 = r47 ? m67 : m45;
+        const int i03 = r03 ? 2 + i23 : i01, i47 = r47 ? 6 + i67 : 4 + i45;
+        const bool r07 = m47 > m03;
+        const float m = r07 ? m47 : m03;
+        const int i = r07 ? i47 : i03;
+        const bool gt = m > best;
+        best = gt ? m : best;
+        k = gt ? g * 8 + i : k;
+    }
+    __device__ __forceinline__ void finish(const EpiTile& t, int lane, float* __restrict__ rec) {
+        const long long p = t.P0 + lane;
+        if (p >= t.n_pix) return;
+        float* r = rec + (long long)t.seg * kPeakFields * t.n_pix + p;
+        r[0 * t.n_pix] = best + nf;                          // NaN marks a segment that saw a non-finite |F|^2
+        r[1 * t.n_pix] = __int_as_float(t.k0 + k);
+    }
+};
+
+// phi-major cubes, vectorised: with one pixel per lane a store instruction moves 4 bytes per lane and needs its own
+// 64-bit address (208 stores and ~450 address instructions per thread and tile).  Here each warp turns a group of
+// eight depths x 32 pixels of FQ and FU around in its own slice of shared memory ([FQ|FU][8 depths][32 pixels],
+// double-buffered, only __syncwarp between the phases) so that lane l holds two consecutive pixels of depths
+// l/16 + {0, 2, 4, 6}: one st.global.cs.v2 writes two full 128-byte lines per warp.  Per group 16 STS + 8 LDS.64 +
+// 8 STG.64.  (Four pixels per lane would halve that again, but 128-bit register quads next to the 64-register TMEM
+// loads and the accumulator pairs make ptxas spill seven accumulator pairs in the drain loop.)
+// Needs n_pix % 2 == 0 and 8-byte aligned cubes (else the scalar path above).  sbuf: this warp's 2 x 512 floats.
+template <bool WITH_SCAN>
+__device__ __forceinline__ void epi_tile_phi_major_vec(const float (&acc)[128], const EpiTile& t, int lane, float* sbuf,
+                                                       float* __restrict__ FQ, float* __restrict__ FU,
+                                                       float* __restrict__ rec) {
+    const int dl = lane >> 4, px = (lane & 15) * 2;             // this lane stores depths dl + {0,2,4,6} of a group, pixels px, px+1
+    const bool pin = t.P0 + px < t.n_pix;                        // n_pix % 2 == 0: both pixels in range or none
+    const long long row0 = (long long)(t.k0 + dl) * t.n_pix + t.P0 + px;
+    float* gq = FQ + row0;
+    float* gu = FU + row0;
+    const long long r2 = 2 * t.n_pix;
+    LightScan sc;
+    if (WITH_SCAN) sc.init();
+#pragma unroll
+    for (int g = 0; g < 7; ++g) {
+        if (g * 8 < t.nv) {                                      // warp-uniform
+            float* b = sbuf + (g & 1) * 512;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                b[e * 32 + lane] = acc[g * 16 + e];
+                b[256 + e * 32 + lane] = acc[g * 16 + 8 + e];
+            }
+            __syncwarp();
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 q = *reinterpret_cast<const float2*>(b + (dl + 2 * i) * 32 + px);
+                const float2 u = *reinterpret_cast<const float2*>(b + 256 + (dl + 2 * i) * 32 + px);
+                if (pin && g * 8 + dl + 2 * i < t.nv) {
+                    __stcs(reinterpret_cast<float2*>(gq), q);
+                    __stcs(reinterpret_cast<float2*>(gu), u);
+                }
+                gq += r2;
+                gu += r2;
+            }
+            if (WITH_SCAN) sc.group(acc, g, t.nv);
+        }
+    }
+    if (WITH_SCAN) sc.finish(t, lane, rec);
+}
+
+// phi-major cubes through a store warp.  One SM stores at most 32 bytes per clock (measured: 106 KB in 3.2 k cycles
+// whatever the vector width and however many SMs store), and inside this kernel, next to ~46 B/clk of inbound TMA
+// traffic, a 106 KB tile took 6.5 k cycles of the epilogue warps' time while the two TMEM accumulator buffers give
+// the MMA issuer only 2.5 k cycles of slack (profiles/r02_tile_timeline_cfg5.txt).  With few channels (few chunks per
+// tile) that stall is a large share of the item, so there the epilogue warps do not store: the four warps of a column half (128 pixels) stage a group of eight depths of FQ and of FU -- two
+// [8 depths][128 pixels] slabs, 8 KB -- in a ring of six such pairs and go back to draining accumulators; a
+// dedicated warp empties the ring with LDS.128 + st.global.cs.v4 (one instruction = one 512-byte row = four full
+// lines) and stalls on the store queue in their stead.  (TMA box stores out of the same ring were measured first:
+// ~1.7 k cycles of latency per store, so the 40 KB in flight drained at 19 B/clk.)
+// Pairs are used in a fixed order known to both sides: per work item, for g = 0..6: [half 0, group g] if g < ng0, then
+// [half 1, group g] if g < ng1.  full[slot]: 4 warp arrivals; empty[slot]: 1 arrival by the store warp.
+constexpr int kRingSlots = 6, kRingSlotFloats = 2048;
+struct TileRing {
+    float* base;          // kRingSlots x 2048 floats
+    uint64_t* full;       // [kRingSlots]
+    uint64_t* empty;      // [kRingSlots]
+    uint32_t seq;         // pairs pushed / popped so far by this thread's role (slot = seq % 6, phase = seq / 6 & 1)
+    __device__ __forceinline__ void init(float* b, uint64_t* f, uint64_t* e) { base = b; full = f; empty = e; seq = 0; }
+};
+// number of 8-depth groups the two column halves hold of a depth tile with nv_tile valid depths
+__device__ __forceinline__ void ring_groups(int nv_tile, int& ng0, int& ng1) {
+    ng0 = (min(nv_tile, 56) + 7) >> 3;
+    ng1 = (max(min(nv_tile - 56, 48), 0) + 7) >> 3;
+}
+
+template <bool WITH_SCAN>
+__device__ __forceinline__ void epi_tile_phi_major_ring(const float (&acc)[128], const EpiTile& t, int lane, int q, int half,
+                                                        int nv_tile, TileRing& ring, float* __restrict__ rec) {
+    int ng0, ng1;
+    ring_groups(nv_tile, ng0, ng1);
+    LightScan sc;
+    if (WITH_SCAN) sc.init();
+#pragma unroll
+    for (int g = 0; g < 7; ++g) {
+        if (g < (half ? ng1 : ng0)) {                            // uniform over the four warps of the half
+            const uint32_t n = ring.seq + (half ? min(g + 1, ng0) + g : g + min(g, ng1));   // position in the item's pair order
+            const uint32_t slot = n % kRingSlots, phase = (n / kRingSlots) & 1u;
+            mbar_wait(&ring.empty[slot], phase ^ 1u);
+            float* b = ring.base + slot * kRingSlotFloats;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                b[e * 128 + q * 32 + lane] = acc[g * 16 + e];
+                b[1024 + e * 128 + q * 32 + lane] = acc[g * 16 + 8 + e];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ring.full[slot]);
+            if (WITH_SCAN) sc.group(acc, g, t.nv);
+        }
+    }
+    ring.seq += ng0 + ng1;
+    if (WITH_SCAN) sc.finish(t, lane, rec);
+}
+
+// The store warp's side: one work item = ng0 + ng1 pairs.  pix_tile: first pixel of the CTA's 128-pixel tile;
+// k_tile: first depth of the depth tile.
+__device__ __forceinline__ void ring_store_item(TileRing& ring, int lane, long long pix_tile, int k_tile, int nv_tile, long long n_pix,
+                                                float* __restrict__ FQ, float* __restrict__ FU) {
+    int ng0, ng1;
+    ring_groups(nv_tile, ng0, ng1);
+    const bool pin = pix_tile + lane * 4 < n_pix;                // n_pix % 4 == 0: four pixels in range or none
+    for (int g = 0; g < 7; ++g) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            if (g >= (half ? ng1 : ng0)) continue;
+            const uint32_t slot = ring.seq % kRingSlots, phase = (ring.seq / kRingSlots) & 1u;
+            ++ring.seq;
+            mbar_wait(&ring.full[slot], phase);
+            const float4* b = reinterpret_cast<const float4*>(ring.base + slot * kRingSlotFloats) + lane;
+            const int d0 = half * 56 + g * 8;                    // first local depth of the pair
+            const long long row = (long long)(k_tile + d0) * n_pix + pix_tile + lane * 4;
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {                        // two depth rows of both cubes per round (the warp has 32 registers)
+                float4 vq[2], vu[2];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) { vq[i] = b[(h * 2 + i) * 32]; vu[i] = b[256 + (h * 2 + i) * 32]; }
+                if (h == 3) {
+                    // the slot goes back as soon as its last rows have ARRIVED in registers (the dummy AND makes the
+                    // arrival wait for them), not when the stores below have found room in the store queue
+                    uint32_t z0, z1;
+                    asm volatile("and.b32 %0, %1, 0;" : "=r"(z0) : "r"(__float_as_uint(vq[1].w)));
+                    asm volatile("and.b32 %0, %1, 0;" : "=r"(z1) : "r"(__float_as_uint(vu[1].w)));
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&ring.empty[slot + z0 + z1]);
+                }
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    if (pin && d0 + h * 2 + i < nv_tile) {
+                        __stcs(reinterpret_cast<float4*>(FQ + row + (h * 2 + i) * n_pix), vq[i]);
+                        __stcs(reinterpret_cast<float4*>(FU + row + (h * 2 + i) * n_pix), vu[i]);
+                    }
+                }
+            }
+        }
+    }
 }
 
 }  // namespace rms

@@ -16,8 +16,6 @@
 //   acc_empty[b] LEADER's: chunk drained by BOTH epilogues    (8 local + 8 remote warp arrivals)
 // Remote arrivals use mbarrier.arrive.shared::cluster with default semantics, as NVIDIA's 2-SM kernels do;
 // a .release.cluster arrival was measured at ~1000 cycles each and starved the MMA thread (50 % idle).
-#include <cstdio>
-#include <cstdlib>
 #include "common.cuh"
 #include "tc_common.cuh"
 #include "tc_epilogue.cuh"
@@ -84,8 +82,9 @@ struct Tc2Params {
     float* FU;
     float* FA;           // |F| cube (Eq. 17), may be NULL
     float* rec;          // peak-segment records (tc_epilogue.cuh), NULL = no peak search
-    int* tile_sync;      // [pixel-tile pairs] check-in counters (tile_checkin), NULL = off
-    long long* prof;
+    int* tile_sync;      // [pixel-tile pairs] check-in counters (gang_checkin), NULL = off
+    int gang;                     // gang size G of the work schedule (tc_common.cuh: WorkIter)
+    int sync_lag;        // gang members may drift this many work items apart
 };
 
 template <int IN_MN, int OUT_LOS>
@@ -135,11 +134,11 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
             int tp, j;
             while (wi.next(tp, j)) {
                 const int pix0 = (2 * tp + (int)rank) * T2_M;       // may lie past n_pix: TMA zero-fills
-                tile_checkin(prm.tile_sync && wi.ganged() ? prm.tile_sync + tp : nullptr, 2 * prm.n_phi_tiles);
+                gang_checkin(prm.tile_sync, wi, tp, prm.sync_lag, 2 * prm.gang);
                 const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) +
                                       ((size_t)j * prm.n_stages * 2 + rank) * 2 * b_part_bytes;
                 for (int s = 0; s < prm.n_stages; ++s) {
@@ -175,24 +174,18 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)IN_MN << 15) |
                                    ((uint32_t)(N2 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
             uint32_t st = 0, ph = 0, ab = 0, aph = 0;
-            long long w_ready = 0, w_acc = 0, t_begin = clock64(), t0 = 0;
-            const bool prof = prm.prof != nullptr;
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
             int tp, j;
             while (wi.next(tp, j))
                 for (int c = 0; c < n_chunks; ++c) {
-                    if (prof) t0 = clock64();
                     mbar_wait(&acc_empty[ab], aph ^ 1);
-                    if (prof) w_acc += clock64() - t0;
                     tc_fence_after();
                     const uint32_t d_tmem = tmem + ab * 256;
                     const int s_end = min(prm.n_stages, (c + 1) * T2_CHUNK_STAGES);
                     uint32_t first = 1;
                     for (int s = c * T2_CHUNK_STAGES; s < s_end; ++s) {
-                        if (prof) t0 = clock64();
                         mbar_wait(&ready[st], ph);
-                        if (prof) w_ready += clock64() - t0;
                         tc_fence_after();
                         const uint32_t sb = smem_base + st * T2_STAGE;
                         const uint32_t aQ = sb, aU = sb + T2_APART, aQl = sb + 2 * T2_APART, aUl = sb + 3 * T2_APART;
@@ -219,10 +212,6 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     __syncwarp();
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
-            if (prof && lead) {
-                prm.prof[cluster_id * 8 + 0] = 0; prm.prof[cluster_id * 8 + 1] = w_ready;
-                prm.prof[cluster_id * 8 + 2] = w_acc; prm.prof[cluster_id * 8 + 3] = clock64() - t_begin;
-            }
         }
         __syncwarp();
       }
@@ -234,7 +223,7 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         long long total = 0;                                 // stages this cluster will see = its work items x n_stages
         {
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
             int tp, j;
             while (wi.next(tp, j)) total += prm.n_stages;
         }
@@ -266,17 +255,13 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         uint32_t ab = 0, aph = 0;
         float acc[128];
-        const bool prof = prm.prof != nullptr && warp == 8 && rank == 0;
-        long long e_wait = 0, e_drain = 0, e_store = 0, e_scan = 0, t0 = 0, t1 = 0;
         WorkIter wi;
-        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
         int tp, j;
         while (wi.next(tp, j)) {
             const long long P0 = (long long)(2 * tp + (int)rank) * T2_M + q * 32;   // first pixel of this warp
             for (int c = 0; c < n_chunks; ++c) {
-                if (prof) t0 = clock64();
                 mbar_wait(&acc_full[ab], aph);
-                if (prof) { t1 = clock64(); e_wait += t1 - t0; }
                 tc_fence_after();
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
@@ -297,9 +282,7 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(mapa_u32(smem_u32(&acc_empty[ab]), 0));
                 if (++ab == 2) { ab = 0; aph ^= 1; }
-                if (prof) e_drain += clock64() - t1;
             }
-            if (prof) t0 = clock64();
             EpiTile et;
             et.n_pix = prm.n_pix;
             et.P0 = P0;
@@ -315,12 +298,6 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 if (!OUT_LOS) epi_tile_phi_major<false>(acc, et, lane, prm.FQ, prm.FU, prm.FA, nullptr);
                 else epi_tile_los_major<false>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, nullptr);
             }
-            if (prof) { t1 = clock64(); e_store += t1 - t0; }
-            if (prof) e_scan += clock64() - t1;
-        }
-        if (prof && lane == 0) {
-            prm.prof[cluster_id * 8 + 4] = e_wait; prm.prof[cluster_id * 8 + 5] = e_drain;
-            prm.prof[cluster_id * 8 + 6] = e_store; prm.prof[cluster_id * 8 + 7] = e_scan;
         }
     }
     tc_fence_before();
@@ -346,7 +323,7 @@ rmsynth_status tc2_plan_init(rmsynth_plan* p) {
 
 rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
                           bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
-                          cudaStream_t st) {
+                          int gang, int sync_lag, cudaStream_t st) {
     Tc2Params prm;
     prm.n_pix = n_pix;
     prm.n_chan = p->n_chan;
@@ -364,15 +341,11 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.FA = FA;
     prm.rec = rec;
     prm.tile_sync = tile_sync;
-    prm.prof = nullptr;
+    prm.gang = gang;
+    prm.sync_lag = sync_lag;
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
     const int grid = 2 * clusters;
-    static const bool want_prof = getenv("RMSYNTH_TC_PROFILE") != nullptr;
-    if (want_prof) {
-        RMS_CUDA(cudaMalloc(&prm.prof, sizeof(long long) * 8 * clusters));
-        RMS_CUDA(cudaMemset(prm.prof, 0, sizeof(long long) * 8 * clusters));
-    }
     const CUtensorMap& mq = *static_cast<const CUtensorMap*>(map_q);
     const CUtensorMap& mu = *static_cast<const CUtensorMap*>(map_u);
     if (in_freq && out_phi) tc2_rmsynth_kernel<1, 0><<<grid, T2_THREADS, T2_SMEM, st>>>(mq, mu, prm);
@@ -380,16 +353,6 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     else if (out_phi) tc2_rmsynth_kernel<0, 0><<<grid, T2_THREADS, T2_SMEM, st>>>(mq, mu, prm);
     else tc2_rmsynth_kernel<0, 1><<<grid, T2_THREADS, T2_SMEM, st>>>(mq, mu, prm);
     RMS_LAUNCH_CHECK("tc2_rmsynth_kernel");
-    if (want_prof) {   // debug only: synchronises
-        std::vector<long long> h(8 * clusters);
-        RMS_CUDA(cudaMemcpy(h.data(), prm.prof, sizeof(long long) * 8 * clusters, cudaMemcpyDeviceToHost));
-        cudaFree(prm.prof);
-        double a[8] = {};
-        for (int i = 0; i < clusters; ++i) for (int j = 0; j < 8; ++j) a[j] += (double)h[8 * i + j] / clusters;
-        fprintf(stderr, "[rmsynth tc2 profile] MMA thread: total %.0f cyc; waiting ready %.1f%% acc_empty %.1f%% | epilogue warp: "
-                "wait %.1f%% drain %.1f%% store %.1f%% scan %.1f%%\n", a[3], 100 * a[1] / a[3], 100 * a[2] / a[3],
-                100 * a[4] / a[3], 100 * a[5] / a[3], 100 * a[6] / a[3], 100 * a[7] / a[3]);
-    }
     return RMSYNTH_OK;
 }
 

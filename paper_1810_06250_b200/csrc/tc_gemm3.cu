@@ -3,13 +3,17 @@
 //
 //   [FQ | FU](256 pixels x 2n depths)  =  Q [Bc | -Bs]  +  U [Bs | Bc],   per CTA pair (cta_group::2, M = 256)
 //
-// Split precision.  kind::f16 multiplies 11-bit significands exactly and honours FP16 subnormals (measured,
-// profiles/r01_probe_f16.txt), so a value scaled into [2^14, 2^15) is carried as hi + lo (two FP16 numbers,
-// 22 significant bits, absolute floor 2^-25): x s = hi + lo,  F = sum (hi_a hi_b + lo_a hi_b + hi_a lo_b).
+// Split precision.  kind::f16 multiplies 11-bit significands exactly and honours FP16 subnormals (measured on the
+// box), so a scaled value is carried as hi + lo (two FP16 numbers):
+//   x s = hi + lo,  F = sum (hi_a hi_b + lo_a hi_b + hi_a lo_b).
 //   * B = K w cos/sin is scaled once at plan time by a power of two (FP64 split).
-//   * Q, U are scaled per (pixel, 32-channel chunk) by a power of two taken from the chunk's largest |sample|
-//     over the channels with w > 0; zero-weight channels are replaced by zeros (they contribute nothing, A13),
-//     so a flagged channel full of interference cannot crush the scale of its neighbours.
+//   * Q, U are scaled per (pixel, 32-channel chunk) by a power of two s that brings the chunk's largest |sample|
+//     over the channels with w > 0 into [2^14, 2^15); zero-weight channels are replaced by zeros (they contribute
+//     nothing, A13), so a flagged channel full of interference cannot crush the scale of its neighbours.
+//     hi = x s rounded to a multiple of 16 (11 bits below 2^15: exact in FP16), lo = x s - hi (|lo| <= 8, exact in
+//     FP32, then rounded to FP16: error <= 2^-9, i.e. 2^-23 of the chunk's largest sample).  Three packed FP32
+//     instructions per PAIR of samples: hi' = fma(x, s, C) with C = 1.5 2^27 (one rounding, to a multiple of 16),
+//     hi = hi' - C, lo = fma(x, s, -hi).
 //   * The TMEM FP32 accumulator is drained after every chunk (12 MMAs) into FP32 registers with
 //     acc += drained * 2^-e(pixel, chunk): the drains the accumulator's round-toward-zero already demands
 //     (tc_gemm2.cu) are what makes a per-chunk scale free.
@@ -21,8 +25,8 @@
 // 16-channel slots at 416 + 32 s: [Q_hi 8 | Q_lo 8 | U_hi 8 | U_lo 8] columns, two FP16 per column.
 //
 // Warps (512 threads, 1 CTA/SM, CTA pairs, persistent over (pixel-tile pair, depth tile) items):
-//   0 raw-tile TMA producer | 1 MMA issuer (leader CTA) | 2 TMEM allocator + B producer | 4-7 transform |
-//   8-15 epilogue (tc_epilogue.cuh: stores in either layout, |F| cube, fused peak search)
+//   0 raw-tile TMA producer | 1 MMA issuer (leader CTA) | 2 TMEM allocator + B producer |
+//   4-11 epilogue (tc_epilogue.cuh: stores in either layout, |F| cube, fused peak search) | 12-15 transform
 #include <cuda.h>
 #include <cuda_fp16.h>
 #include <cstdio>
@@ -43,9 +47,12 @@ constexpr int T3_SCALES = 8;                     // ring of per-pixel chunk scal
 constexpr int T3_ACC_COLS = 208, T3_A_COL0 = 416;
 constexpr int T3_OFF_B = T3_R * T3_RAW;
 constexpr int T3_OFF_SCALE = T3_OFF_B + T3_S * T3_BSTAGE;
-constexpr int T3_OFF_BARS = T3_OFF_SCALE + T3_SCALES * T3_M * 4;
+constexpr int T3_OFF_BARS = T3_OFF_SCALE + T3_SCALES * T3_M * 2;   // scales are powers of two: kept as bf16 bit patterns
+constexpr int T3_MASKS = 48;                     // channel masks of the first 48 chunks live in shared memory
+constexpr int T3_OFF_MASK = T3_OFF_BARS + 320;   // 34 barriers + the TMEM address word come first
 constexpr int T3_OFF_STAGE_T = T3_OFF_BARS + 512;
-constexpr int T3_SMEM_PHI = T3_OFF_STAGE_T + 1024;                    // + alignment slack
+constexpr int T3_SMEM_PHI = T3_OFF_STAGE_T + kRingSlots * 8192 + 1024; // output ring (6 pairs x 8 KB) + alignment slack
+static_assert(T3_SMEM_PHI <= 227 * 1024, "shared memory budget");
 constexpr int T3_SMEM_LOS = T3_OFF_STAGE_T + 8 * 32 * 33 * 4 + 1024;
 constexpr int T3_THREADS = 512;
 static_assert(T3_SMEM_LOS <= 227 * 1024, "shared memory budget");
@@ -116,7 +123,11 @@ struct Tc3Params {
     float* FU;
     float* FA;                    // |F| cube, may be NULL
     float* rec;                   // peak-segment records, NULL = no peak search
-    int* tile_sync;               // [pixel-tile pairs] check-in counters (tile_checkin), NULL = off
+    int* tile_sync;               // [pixel-tile pairs] check-in counters (gang_checkin), NULL = off
+    int gang;                     // gang size G of the work schedule (tc_common.cuh: WorkIter)
+    int sync_lag;                 // gang members may drift this many work items apart
+    int stagger;                  // cycles by which consecutive gangs delay their start (de-phases the tile-end store bursts)
+    long long* tl;                // timeline buffer (debug build), else NULL
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -138,22 +149,52 @@ __device__ __forceinline__ void t3_load_raw(const uint8_t* raw, int row, bool in
     }
 }
 
-// hi = t truncated to 11 significant bits (exact in FP16 unless subnormal there), lo = t - hi; two channels per register
-__device__ __forceinline__ void t3_split(float x0, float x1, float scale, uint32_t& hi, uint32_t& lo) {
-    const float t0 = x0 * scale, t1 = x1 * scale;
-    const float h0 = __uint_as_float(__float_as_uint(t0) & 0xFFFFE000u), h1 = __uint_as_float(__float_as_uint(t1) & 0xFFFFE000u);
-    const __half2 h = __floats2half2_rn(h0, h1), l = __floats2half2_rn(t0 - h0, t1 - h1);
-    hi = *reinterpret_cast<const uint32_t*>(&h);
-    lo = *reinterpret_cast<const uint32_t*>(&l);
+// Packed FP32 arithmetic (sm_100: FFMA2 / FADD2 work on register pairs; one issue slot for two lanes of work).
+__device__ __forceinline__ uint64_t pack2(float a, float b) {
+    uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+    uint64_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+    uint64_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
-template <int IN_MN, int OUT_LOS>
+// Two channels per call: hi = x s rounded to a multiple of 16 (exact in FP16 for |x s| < 2^15), lo = x s - hi.
+__device__ __forceinline__ void t3_split(float x0, float x1, uint64_t scale2, uint32_t& hi, uint32_t& lo) {
+    constexpr float C = 201326592.f;                         // 1.5 2^27: ulp 16
+    const uint64_t x = pack2(x0, x1);
+    const uint64_t h = add2(fma2(x, scale2, pack2(C, C)), pack2(-C, -C));
+    float h0, h1, l0, l1;
+    unpack2(h, h0, h1);
+    unpack2(fma2(x, scale2, pack2(-h0, -h1)), l0, l1);
+    const __half2 hh = __floats2half2_rn(h0, h1), ll = __floats2half2_rn(l0, l1);
+    hi = *reinterpret_cast<const uint32_t*>(&hh);
+    lo = *reinterpret_cast<const uint32_t*>(&ll);
+}
+
+// acc2[0..N/2) += drained[0..N) * inv: the accumulators live as register PAIRS, two columns per FFMA2
+template <int N>
+__device__ __forceinline__ void t3_accumulate(uint64_t* acc2, const uint32_t* r, uint64_t inv2) {
+#pragma unroll
+    for (int i = 0; i < N / 2; ++i)
+        asm("{\n.reg .b64 t;\nmov.b64 t, {%1, %2};\nfma.rn.f32x2 %0, t, %3, %0;\n}" : "+l"(acc2[i]) : "r"(r[2 * i]), "r"(r[2 * i + 1]), "l"(inv2));
+}
+
+// OUT: 0 = phi-major cubes, scalar stores (any shape; also |F| cube and maps-only calls), 1 = LOS-major cubes,
+//      2 = phi-major through the output ring and the store warp, 3 = phi-major, vectorised stores (tc_epilogue.cuh)
+template <int IN_MN, int OUT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
 tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU, const Tc3Params prm) {
+    constexpr bool OUT_LOS = OUT == 1;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    float* scales = reinterpret_cast<float*>(smem_gen + T3_OFF_SCALE);            // [T3_SCALES][128]
+    uint16_t* scales = reinterpret_cast<uint16_t*>(smem_gen + T3_OFF_SCALE);      // [T3_SCALES][128] upper halves of FP32 powers of two
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_gen + T3_OFF_BARS);
     uint64_t* raw_full = bars;                    // [R] raw tile landed                     (1 + tx)
     uint64_t* raw_empty = raw_full + T3_R;        // [R] raw tile read by the transform      (4 warps)
@@ -163,7 +204,10 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     uint64_t* a_empty = a_ready + T3_NA;          // [NA] MMAs that read the slot done        (multicast commit)
     uint64_t* acc_full = a_empty + T3_NA;         // [2] chunk accumulated, both CTAs         (multicast commit)
     uint64_t* acc_empty = acc_full + 2;           // [2] LEADER's: chunk drained by both epilogues (8 + 8 warps)
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+    uint64_t* ring_full = acc_empty + 2;          // [6] output pair staged                           (4 epilogue warps)
+    uint64_t* ring_empty = ring_full + kRingSlots; // [6] output pair read by the store warp          (1)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ring_empty + kRingSlots);
+    uint32_t* smask = reinterpret_cast<uint32_t*>(smem_gen + T3_OFF_MASK);        // [T3_MASKS]
     float* stage_t = reinterpret_cast<float*>(smem_gen + T3_OFF_STAGE_T);         // LOS-major transpose buffers
 
     // warp index through a shuffle: provably warp-uniform, so role branches are uniform and MMA operands stay in uniform registers
@@ -179,8 +223,11 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         for (int s = 0; s < T3_S; ++s) { mbar_init(&b_full[s], 1); mbar_init(&b_empty[s], 1); }
         for (int s = 0; s < T3_NA; ++s) { mbar_init(&a_ready[s], 8); mbar_init(&a_empty[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], 16); }
+        for (int s = 0; s < kRingSlots; ++s) { mbar_init(&ring_full[s], 4); mbar_init(&ring_empty[s], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (threadIdx.x >= 64 && threadIdx.x < 64 + T3_MASKS)   // T3_MASKS <= 64
+        smask[threadIdx.x - 64] = (int)threadIdx.x - 64 < n_chunks ? prm.chan_mask[threadIdx.x - 64] : 0u;
     if (warp == 2) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
@@ -197,14 +244,31 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         if (lane == 0) {
             const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
+            TlRole tl;
+            tl.init(prm.tl, TL_PRODUCER);
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
+            // Every work item costs the same, so CTAs that start together reach their tile ends together and all 148
+            // SMs store their 106 KB tiles at the same moment: 15.7 MB at the ~3.8 TB/s the memory system absorbs is
+            // ~6.5 k cycles during which no epilogue warp drains (measured, profiles/r02_tile_timeline_cfg5.txt), then
+            // nobody writes for the rest of the item.  Gang g therefore starts g x stagger cycles late; the phases then
+            // stay spread over the item period and a tile's stores find the memory system idle.
+            if (prm.stagger > 0) {
+                const int G = prm.gang, S = (n_clusters / G) * G;
+                const long long wait = (long long)(cluster_id < S ? cluster_id / G : S / G + cluster_id - S) * prm.stagger;
+                const long long t0 = clock64();
+                while (clock64() - t0 < wait) __nanosleep(64);
+            }
             int tp, j;
             while (wi.next(tp, j)) {
                 const int pix0 = (2 * tp + (int)rank) * T3_M;       // may lie past n_pix: TMA zero-fills
-                tile_checkin(prm.tile_sync && wi.ganged() ? prm.tile_sync + tp : nullptr, 2 * prm.n_phi_tiles);
+                tl.stamp(0);
+                gang_checkin(prm.tile_sync, wi, tp, prm.sync_lag, 2 * prm.gang);
+                tl.stamp(1);
                 for (int c = 0; c < n_chunks; ++c) {
+                    tl.begin();
                     mbar_wait(&raw_empty[st], ph ^ 1);
+                    tl.add(3);
                     mbar_expect_tx(&raw_full[st], T3_RAW);
                     const uint32_t sb = smem_base + st * T3_RAW;
                     if (IN_MN) {
@@ -224,6 +288,8 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     }
                     if (++st == T3_R) { st = 0; ph ^= 1; }
                 }
+                tl.stamp(2);
+                tl.next();
             }
         }
         __syncwarp();
@@ -233,7 +299,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const uint64_t pol = l2_policy_evict_last();
             uint32_t st = 0, ph = 0;
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
             int tp, j;
             while (wi.next(tp, j)) {
                 const uint8_t* bsrc = reinterpret_cast<const uint8_t*>(prm.blob) + ((size_t)j * n_chunks * 2 + rank) * b_bytes;
@@ -261,18 +327,25 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             const uint64_t dhi = make_desc(0u, 16u * n, 128u, 0u);
             const uint32_t o_part = (128u * n) >> 4, o_slot = (64u * n) >> 4, o_ks = (32u * n) >> 4;
             uint32_t sa = 0, pa = 0, sb = 0, ab = 0, aph = 0;
+            TlRole tl;
+            tl.init(prm.tl, TL_ISSUER);
             WorkIter wi;
-            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
             int tp, j;
-            while (wi.next(tp, j))
+            while (wi.next(tp, j)) {
+                tl.stamp(0);
                 for (int c = 0; c < n_chunks; ++c) {
+                    tl.begin();
                     mbar_wait(&acc_empty[ab], aph ^ 1);
+                    tl.add(c < 2 ? 4 : 1);                 // slot 4: the first two chunks of an item (the tile-end bubble)
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_u + ab * T3_ACC_COLS;
                     const uint32_t baddr = (smem_u + T3_OFF_B + sb * T3_BSTAGE) >> 4;
 #pragma unroll
                     for (int ks = 0; ks < 2; ++ks) {
+                        tl.begin();
                         mbar_wait(&a_ready[sa], pa);       // A slot written and (ks == 0) B chunk landed, in both CTAs
+                        tl.add(c == 0 && ks == 0 ? 5 : 2); // slot 5: the first A slot of an item
                         tc_fence_after();
                         const uint32_t a0 = tmem_u + T3_A_COL0 + sa * 32;
                         const uint64_t d0 = dhi | (uint64_t)(baddr + ks * o_ks);             // hi part, slot 0
@@ -293,25 +366,44 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     if (++sb == T3_S) sb = 0;
                     if (++ab == 2) { ab = 0; aph ^= 1; }
                 }
+                tl.stamp(3);
+                tl.next();
+            }
         }
         __syncwarp();
+      } else if (OUT == 2) {
+        // ===================== store warp (both CTAs): output ring -> global (tc_epilogue.cuh) =====================
+        TileRing ring;
+        ring.init(stage_t, ring_full, ring_empty);
+        WorkIter wi;
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
+        int tp, j;
+        while (wi.next(tp, j))
+            ring_store_item(ring, lane, (long long)(2 * tp + (int)rank) * T3_M, j * n, min(n, prm.n_phi - j * n), prm.n_pix, prm.FQ, prm.FU);
       }
-    } else if (warp < 8) {
+    } else if (warp >= 12) {
         // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
+        // The highest warp ids: the scheduler favours them over the epilogue warps of the same sub-partition, and this
+        // role is the latency-critical one (the MMA issuer waits for every A slot; the epilogue has slack).
         asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        const int row = threadIdx.x - 128;                          // pixel row of the tile = TMEM lane
+        const int row = threadIdx.x - 384;                          // pixel row of the tile = TMEM lane
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         uint32_t sr = 0, pr = 0, sa = 0, pa = 0, sb = 0, pb = 0, seq = 0;
         const uint32_t ready0 = mapa_u32(smem_u32(&a_ready[0]), 0);
+        TlRole tl;
+        tl.init(warp == 12 ? prm.tl : nullptr, TL_TRANSFORM);
         WorkIter wi;
-        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
         int tp, j;
         while (wi.next(tp, j)) {
+            tl.stamp(0);
             for (int c = 0; c < n_chunks; ++c) {
                 float v[64];
+                tl.begin();
                 mbar_wait(&raw_full[sr], pr);
+                tl.lap(c == 0 ? 5 : 1);
                 t3_load_raw(smem_gen + sr * T3_RAW, row, IN_MN, v);
-                const uint32_t mask = __ldg(prm.chan_mask + c);
+                const uint32_t mask = c < T3_MASKS ? smask[c] : __ldg(prm.chan_mask + c);
                 if (mask != 0xFFFFFFFFu) {                          // warp-uniform: zero the zero-weight channels
 #pragma unroll
                     for (int i = 0; i < 32; ++i)
@@ -328,34 +420,59 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 int e = (int)(__float_as_uint(m) >> 23);
                 e = min(max(e, 15), 254);
                 const float scale = __uint_as_float((uint32_t)(268 - e) << 23);
-                scales[(seq & (T3_SCALES - 1)) * T3_M + row] = __uint_as_float((uint32_t)(e - 14) << 23);   // 2^(e - 141)
+                const uint64_t scale2 = pack2(scale, scale);
+                // what the epilogue multiplies the drained chunk with: 2^(e - 141) 2^-eB (B's plan-time scale folded in)
+                scales[(seq & (T3_SCALES - 1)) * T3_M + row] =
+                    (uint16_t)(__float_as_uint(__uint_as_float((uint32_t)(e - 14) << 23) * prm.inv_scale_b) >> 16);
                 ++seq;
-                // Both 16-channel slots are written before the one tcgen05.wait::st: the second conversion overlaps the
-                // first store, and the chunk pays one store round trip instead of two.
+                // The two 16-channel slots are published separately.  The first slot of a chunk was released long ago
+                // (by the chunk before the previous one), the second only half-way through the previous chunk's MMAs:
+                // published together, the chain  commit -> a_empty -> tcgen05.st -> wait::st -> remote arrive -> issuer
+                // (~800 cycles) had to fit into the 624 cycles the previous chunk's second K step lasts, and the tensor
+                // pipe idled ~250 cycles per chunk (profiles/r02_tile_timeline_cfg5.txt).  Published separately, the
+                // first K step never waits for it and the second has a whole K step more of slack.
                 const uint32_t s0 = sa, s1 = sa + 1 == T3_NA ? 0 : sa + 1;
                 const uint32_t p0 = pa, p1 = sa + 1 == T3_NA ? pa ^ 1 : pa;
+                uint32_t r0[32], r1[32];
 #pragma unroll
-                for (int ks = 0; ks < 2; ++ks) {
-                    uint32_t r[32];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        t3_split(v[ks * 16 + 2 * i], v[ks * 16 + 2 * i + 1], scale, r[i], r[8 + i]);
-                        t3_split(v[32 + ks * 16 + 2 * i], v[32 + ks * 16 + 2 * i + 1], scale, r[16 + i], r[24 + i]);
-                    }
-                    mbar_wait(&a_empty[ks ? s1 : s0], (ks ? p1 : p0) ^ 1);
-                    tc_fence_after();
-                    tmem_st32(tmem + lane_addr + T3_A_COL0 + (ks ? s1 : s0) * 32, r);
+                for (int i = 0; i < 8; ++i) {
+                    t3_split(v[2 * i], v[2 * i + 1], scale2, r0[i], r0[8 + i]);
+                    t3_split(v[32 + 2 * i], v[32 + 2 * i + 1], scale2, r0[16 + i], r0[24 + i]);
                 }
+                tl.lap(6);                                           // loads, chunk maximum, split arithmetic
+                mbar_wait(&a_empty[s0], p0 ^ 1);
+                tl.lap(2);
+                tc_fence_after();
+                tmem_st32(tmem + lane_addr + T3_A_COL0 + s0 * 32, r0);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {                        // the second conversion overlaps the first store
+                    t3_split(v[16 + 2 * i], v[16 + 2 * i + 1], scale2, r1[i], r1[8 + i]);
+                    t3_split(v[48 + 2 * i], v[48 + 2 * i + 1], scale2, r1[16 + i], r1[24 + i]);
+                }
+                tl.lap(6);
                 tmem_st_wait();
+                tl.lap(7);                                           // TMEM store round trip
                 mbar_wait(&b_full[sb], pb);                          // the B chunk of this CTA must have landed too
+                tl.lap(3);
                 if (++sb == T3_S) { sb = 0; pb ^= 1; }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) { mbar_arrive_remote(ready0 + s0 * 8); mbar_arrive_remote(ready0 + s1 * 8); }
+                if (lane == 0) mbar_arrive_remote(ready0 + s0 * 8);
+                mbar_wait(&a_empty[s1], p1 ^ 1);
+                tl.lap(2);
+                tc_fence_after();
+                tmem_st32(tmem + lane_addr + T3_A_COL0 + s1 * 32, r1);
+                tmem_st_wait();
+                tl.lap(7);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(ready0 + s1 * 8);
                 pa = p1;
                 sa = s1 + 1 == T3_NA ? 0 : s1 + 1;
                 if (sa == 0) pa ^= 1;
             }
+            tl.stamp(4);
+            tl.next();
         }
     } else {
         // ===================== epilogue (both CTAs, own TMEM lanes = own 128 pixels) =====================
@@ -363,66 +480,61 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const int q = warp & 3;
         // Columns are split 112 / 96 (7 / 6 depth groups) between the two warps of a lane quarter, so that 64 staging
         // registers fit next to the accumulators and a drain is two TMEM load round trips (~230 cycles each) instead of four.
-        const int half = warp >= 12 ? 1 : 0;
+        const int half = warp >= 8 ? 1 : 0;
         const int cbase = half ? 112 : 0;
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t empty0 = mapa_u32(smem_u32(&acc_empty[0]), 0);
         uint32_t ab = 0, aph = 0, seq = 0;
-        float acc[128];                                             // 112 (half 0) or 96 (half 1) in use
+        uint64_t acc2[64];                                          // column pairs; 56 (half 0) or 48 (half 1) in use
+        TileRing ring;
+        ring.init(stage_t, ring_full, ring_empty);
+        TlRole tl;
+        tl.init(warp == 4 || warp == 8 ? prm.tl : nullptr, warp == 4 ? TL_EPI0 : TL_EPI1);
         WorkIter wi;
-        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs);
+        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
         int tp, j;
         while (wi.next(tp, j)) {
-            const long long P0 = (long long)(2 * tp + (int)rank) * T3_M + q * 32;   // first pixel of this warp
+            tl.stamp(0);
+#pragma unroll
+            for (int i = 0; i < 64; ++i) acc2[i] = 0ull;
             for (int c = 0; c < n_chunks; ++c) {
+                tl.begin();
                 mbar_wait(&acc_full[ab], aph);
+                tl.add(c == 0 ? 4 : 1);
                 tc_fence_after();
-                const float inv = scales[(seq & (T3_SCALES - 1)) * T3_M + q * 32 + lane];   // 2^-e of this pixel's chunk
+                const float inv = __uint_as_float((uint32_t)scales[(seq & (T3_SCALES - 1)) * T3_M + q * 32 + lane] << 16);   // 2^-e of this pixel's chunk, times 2^-eB
+                const uint64_t inv2 = pack2(inv, inv);
                 ++seq;
                 const uint32_t tbase = tmem + lane_addr + ab * T3_ACC_COLS + cbase;
                 {
                     uint32_t r[64];
                     tmem_ld64(tbase, r);
                     tmem_ld_wait();
-                    if (c == 0) {
-#pragma unroll
-                        for (int i = 0; i < 64; ++i) acc[i] = __uint_as_float(r[i]) * inv;
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 64; ++i) acc[i] = fmaf(__uint_as_float(r[i]), inv, acc[i]);
-                    }
+                    t3_accumulate<64>(acc2, r, inv2);
                 }
                 if (!half) {
                     uint32_t r[48];
                     tmem_ld32(tbase + 64, r);
                     tmem_ld16(tbase + 96, r + 32);
                     tmem_ld_wait();
-                    if (c == 0) {
-#pragma unroll
-                        for (int i = 0; i < 48; ++i) acc[64 + i] = __uint_as_float(r[i]) * inv;
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 48; ++i) acc[64 + i] = fmaf(__uint_as_float(r[i]), inv, acc[64 + i]);
-                    }
+                    t3_accumulate<48>(acc2 + 32, r, inv2);
                 } else {
                     uint32_t r[32];
                     tmem_ld32(tbase + 64, r);
                     tmem_ld_wait();
-                    if (c == 0) {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) acc[64 + i] = __uint_as_float(r[i]) * inv;
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) acc[64 + i] = fmaf(__uint_as_float(r[i]), inv, acc[64 + i]);
-                    }
+                    t3_accumulate<32>(acc2 + 32, r, inv2);
                 }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(empty0 + ab * 8);
                 if (++ab == 2) { ab = 0; aph ^= 1; }
             }
+            tl.stamp(2);
+            float acc[128];
 #pragma unroll
-            for (int i = 0; i < 112; ++i) acc[i] *= prm.inv_scale_b;
+            for (int i = 0; i < 64; ++i) unpack2(acc2[i], acc[2 * i], acc[2 * i + 1]);
+            asm volatile("" : "+r"(tp), "+r"(j));       // keep the tile-end address arithmetic out of the drain loop's live ranges
+            const long long P0 = (long long)(2 * tp + (int)rank) * T3_M + q * 32;   // first pixel of this warp
             EpiTile et;
             et.n_pix = prm.n_pix;
             et.P0 = P0;
@@ -430,14 +542,24 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             et.k0 = j * n + (cbase >> 1);
             et.nv = min(min(n, prm.n_phi - j * n) - (cbase >> 1), half ? 48 : 56);
             et.seg = 2 * j + half;
-            float* sT = stage_t + (warp - 8) * (32 * 33);
-            if (prm.rec) {
+            float* sT = stage_t + (warp - 4) * (32 * 33);
+            if (OUT == 2) {
+                const int nv_tile = min(n, prm.n_phi - j * n);
+                if (prm.rec) epi_tile_phi_major_ring<true>(acc, et, lane, q, half, nv_tile, ring, prm.rec);
+                else epi_tile_phi_major_ring<false>(acc, et, lane, q, half, nv_tile, ring, nullptr);
+            } else if (OUT == 3) {
+                float* sV = stage_t + (warp - 4) * 1024;
+                if (prm.rec) epi_tile_phi_major_vec<true>(acc, et, lane, sV, prm.FQ, prm.FU, prm.rec);
+                else epi_tile_phi_major_vec<false>(acc, et, lane, sV, prm.FQ, prm.FU, nullptr);
+            } else if (prm.rec) {
                 if (!OUT_LOS) epi_tile_phi_major<true>(acc, et, lane, prm.FQ, prm.FU, prm.FA, prm.rec);
                 else epi_tile_los_major<true>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, prm.rec);
             } else {
                 if (!OUT_LOS) epi_tile_phi_major<false>(acc, et, lane, prm.FQ, prm.FU, prm.FA, nullptr);
                 else epi_tile_los_major<false>(acc, et, lane, sT, prm.FQ, prm.FU, prm.FA, nullptr);
             }
+            tl.stamp(3);
+            tl.next();
         }
     }
     tc_fence_before();
@@ -447,6 +569,18 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 
 // ------------------------------------------------------------------------------------------------
 // Host side
+#ifdef RMSYNTH_TIMELINE
+static long long* g_tl_buf = nullptr;
+constexpr size_t kTlCount = (size_t)TL_CTAS * TL_ROLES * TL_ITEMS * TL_SLOTS;
+// Debug build only (not part of include/rmsynth.h): copy out the timeline of the last tc3 launch; synchronises.
+extern "C" int rmsynth_timeline_read(long long* out, int max_count) {
+    if (!g_tl_buf || !out || max_count < (int)kTlCount) return -1;
+    if (cudaDeviceSynchronize() != cudaSuccess) return -2;
+    if (cudaMemcpy(out, g_tl_buf, kTlCount * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) return -3;
+    return (int)kTlCount;
+}
+#endif
+
 rmsynth_status tc3_plan_init(rmsynth_plan* p) {
     TcGeom& g = p->tc3;
     g.kb = T3_KC;
@@ -473,16 +607,16 @@ rmsynth_status tc3_plan_init(rmsynth_plan* p) {
     tc3_build_b_kernel<<<grid, 64>>>(p->d_delta, p->d_kw, p->d_phi, p->n_chan, p->n_phi, g.n_tile, n_chunks,
                                      std::ldexp(1.0, p->tc3_eb), reinterpret_cast<__half*>(p->d_tcB3));
     RMS_LAUNCH_CHECK("tc3_build_b_kernel");
-    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_PHI));
-    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_PHI));
-    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_LOS));
-    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_LOS));
+#define T3_ATTR(IN, O, BYTES) RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<IN, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES))
+    T3_ATTR(0, 0, T3_SMEM_PHI); T3_ATTR(1, 0, T3_SMEM_PHI); T3_ATTR(0, 1, T3_SMEM_LOS); T3_ATTR(1, 1, T3_SMEM_LOS);
+    T3_ATTR(0, 2, T3_SMEM_PHI); T3_ATTR(1, 2, T3_SMEM_PHI); T3_ATTR(0, 3, T3_SMEM_PHI); T3_ATTR(1, 3, T3_SMEM_PHI);
+#undef T3_ATTR
     return RMSYNTH_OK;
 }
 
-rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq,
-                          bool out_phi, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync,
-                          cudaStream_t st) {
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq, bool out_phi,
+                          int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
+                          int sync_lag, cudaStream_t st) {
     Tc3Params prm;
     prm.n_pix = n_pix;
     prm.n_chan = p->n_chan;
@@ -502,15 +636,41 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.FA = FA;
     prm.rec = rec;
     prm.tile_sync = tile_sync;
+    prm.gang = gang;
+    prm.sync_lag = sync_lag;
+    {
+        // one item lasts ~ n_chunks x 1350 cycles (12 MMAs of 104 cycles + overheads); spread the gangs over one item
+        const int max_cl = p->sm_count / 2;
+        const int S = (max_cl / gang) * gang, n_groups = S / gang + (max_cl - S);
+        const char* e = getenv("RMSYNTH_STAGGER");             // EXPERIMENT knob: percent of the default, 0 = off
+        const double scale = e ? atof(e) / 100.0 : 1.0;
+        prm.stagger = (FQ || FA) && n_groups > 1 ? (int)(scale * prm.n_chunks * 1350.0 / n_groups) : 0;
+    }
+    prm.tl = nullptr;
+#ifdef RMSYNTH_TIMELINE
+    if (!g_tl_buf) RMS_CUDA(cudaMalloc(&g_tl_buf, kTlCount * sizeof(long long)));
+    RMS_CUDA(cudaMemsetAsync(g_tl_buf, 0, kTlCount * sizeof(long long), st));
+    prm.tl = g_tl_buf;
+#endif
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
     const int grid = 2 * clusters;
     const CUtensorMap& mq = *static_cast<const CUtensorMap*>(map_q);
     const CUtensorMap& mu = *static_cast<const CUtensorMap*>(map_u);
-    if (in_freq && out_phi) tc3_rmsynth_kernel<1, 0><<<grid, T3_THREADS, T3_SMEM_PHI, st>>>(mq, mu, prm);
-    else if (in_freq) tc3_rmsynth_kernel<1, 1><<<grid, T3_THREADS, T3_SMEM_LOS, st>>>(mq, mu, prm);
-    else if (out_phi) tc3_rmsynth_kernel<0, 0><<<grid, T3_THREADS, T3_SMEM_PHI, st>>>(mq, mu, prm);
-    else tc3_rmsynth_kernel<0, 1><<<grid, T3_THREADS, T3_SMEM_LOS, st>>>(mq, mu, prm);
+    const int out = !out_phi ? 1 : ring_out == 1 ? 2 : ring_out == 2 ? 3 : 0;
+    const int smem = out == 1 ? T3_SMEM_LOS : T3_SMEM_PHI;
+#define T3_LAUNCH(IN, O) tc3_rmsynth_kernel<IN, O><<<grid, T3_THREADS, smem, st>>>(mq, mu, prm)
+    switch (out * 2 + (in_freq ? 1 : 0)) {
+        case 0: T3_LAUNCH(0, 0); break;
+        case 1: T3_LAUNCH(1, 0); break;
+        case 2: T3_LAUNCH(0, 1); break;
+        case 3: T3_LAUNCH(1, 1); break;
+        case 4: T3_LAUNCH(0, 2); break;
+        case 5: T3_LAUNCH(1, 2); break;
+        case 6: T3_LAUNCH(0, 3); break;
+        default: T3_LAUNCH(1, 3); break;
+    }
+#undef T3_LAUNCH
     RMS_LAUNCH_CHECK("tc3_rmsynth_kernel");
     return RMSYNTH_OK;
 }

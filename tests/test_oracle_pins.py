@@ -107,6 +107,29 @@ def test_p5_weighted_mean_lambda0_kills_first_derivative(oracle_mod):
     assert oracle_mod.make_plan(nu, w, [0.0], lambda0_mode=2, lambda0_in=0.0).lambda0_sq == 0.0
 
 
+def test_lambda0_modes_by_value(oracle_mod):
+    """P:L119 "set to the mean of lambda_i^2", reading A2: mode 0 = weighted mean, mode 1 = plain mean over ALL
+    channels (flagged ones included), mode 2 = the caller's value.  Values formed here from c/nu with numpy and
+    with exact rational weights, on a grid where the two means differ in the second digit.
+    Catches: mode 1 silently returning the weighted mean, or a mean over the unflagged channels only."""
+    nu = np.array([100e6, 125e6, 150e6, 200e6])
+    w = np.array([1.0, 0.0, 1.0, 2.0])
+    lam2 = (C / nu) ** 2
+    weighted = (lam2[0] + lam2[2] + 2.0 * lam2[3]) / 4.0           # 4.369
+    plain = lam2.sum() / 4.0                                       # 5.245
+    unflagged_plain = (lam2[0] + lam2[2] + lam2[3]) / 3.0          # 5.076
+    assert abs(weighted - plain) > 0.03 * plain and abs(unflagged_plain - plain) > 0.03 * plain
+    K0, l0 = oracle_mod.plan_scalars(lam2, w, 0)
+    K1, l1 = oracle_mod.plan_scalars(lam2, w, 1)
+    K2, l2 = oracle_mod.plan_scalars(lam2, w, 2, 1.25)
+    assert K0 == K1 == K2 == 0.25                                  # Eq. 13 with sum w = 4, exact
+    assert abs(l0 - weighted) <= 1e-15 * weighted
+    assert abs(l1 - plain) <= 1e-15 * plain
+    assert l2 == 1.25
+    # lambda^2 itself by value: nu = 100 MHz -> lambda = 2.99792458 m
+    assert abs(oracle_mod.lambda_sq(np.array([100e6]))[0] - 2.99792458 ** 2) < 1e-14
+
+
 def test_p6_dirichlet_kernel_closed_form(oracle_mod):
     """Uniform lambda^2 sampling, unit weights: R(phi) = sin(N phi d)/(N sin(phi d)), purely real.
     Catches: dropped factor 2 in the exponent, off-by-one in the channel sum."""
@@ -269,6 +292,36 @@ def test_p12_pa_recovery_for_on_grid_point_source(oracle_mod):
     assert abs(r["peak_phi"][0] - phi0) < 1e-6 and abs(r["peak_amp"][0] - A) < 1e-6
     assert abs(r["pa_zero"][0] - chi0) < 1e-6
     assert -np.pi / 2 <= r["pa_zero"][0] < np.pi / 2
+
+
+def test_p12_pa_zero_wraps_to_half_open_interval(oracle_mod):
+    """Reading A9: pa_zero = pa_lambda0 - phi_peak lambda_0^2 wrapped to [-pi/2, pi/2) (polarisation angles are
+    defined mod pi).  A one-depth grid makes phi_peak = phi[0], so the wrapped argument is known in closed form;
+    expected values are written out as numbers on both sides of +-pi/2, after one and after several turns.
+    Catches: wrapping mod 2 pi, a closed upper end, a sign error for negative arguments."""
+    nu = np.array([150e6, 150e6])                      # lambda_0^2 = (c/150 MHz)^2 exactly, whatever the weights
+    l0 = (C / 150e6) ** 2
+    cases = [  # (pa_lambda0, rotation phi*l0, expected pa_zero)
+        (0.6, 1.0, -0.4),                              # no wrap
+        (-0.7, 1.0, -1.7 + np.pi),                     # below -pi/2 -> + pi  = 1.4415926535897931
+        (1.5, -0.2, 1.7 - np.pi),                      # above +pi/2 -> - pi  = -1.4415926535897931
+        (0.25, 10.0, 0.25 - 10.0 + 3 * np.pi),         # several turns        = -0.3252220392306207
+        (-0.25, -10.0, -0.25 + 10.0 - 3 * np.pi),      #                      = 0.3252220392306207
+        (0.0, -np.pi / 2, -np.pi / 2),                 # +pi/2 exactly maps to the closed lower end
+    ]
+    assert abs(cases[1][2] - 1.4415926535897931) < 1e-15 and abs(cases[3][2] + 0.3252220392306207) < 1e-14
+    for pa, rot, want in cases:
+        plan = oracle_mod.make_plan(nu, None, [rot / l0])
+        assert abs(plan.lambda0_sq - l0) < 1e-15
+        FQ, FU = np.array([[np.cos(2 * pa)]]), np.array([[np.sin(2 * pa)]])
+        r = oracle_mod.peaks(plan, FQ, FU)
+        assert abs(r["pa_lambda0"][0] - pa) < 1e-15
+        assert abs(r["pa_zero"][0] - want) < 1e-13, (pa, rot, r["pa_zero"][0], want)
+        assert -np.pi / 2 <= r["pa_zero"][0] < np.pi / 2
+    # four-quadrant arctangent (A9 "atan2 for tan^-1(U/Q)"): Q < 0 must not fold onto Q > 0
+    plan = oracle_mod.make_plan(nu, None, [0.0])
+    r = oracle_mod.peaks(plan, np.array([[-1.0], [-1.0]]), np.array([[1e-9], [-1e-9]]))
+    assert abs(r["pa_lambda0"][0] - np.pi / 2) < 1e-8 and abs(r["pa_lambda0"][1] + np.pi / 2) < 1e-8
 
 
 # ---------------------------------------------------------------- P13: slab generator
