@@ -86,7 +86,10 @@ void oracle_rmsf(const double *lam2, const double *w, int n_chan,
  *   FU[p,k] = K sum_i w_i ( U[p,i] cos th_ik - Q[p,i] sin th_ik )
  *   th_ik   = 2 phi_k (lambda_i^2 - lambda_0^2)
  * Literal form: cos/sin evaluated inside the innermost loop, channel order,
- * plain FP64 accumulation.  Q,U are the FP32 samples promoted to FP64 (A12). */
+ * plain FP64 accumulation.  Q,U are the FP32 samples promoted to FP64 (A12).
+ * Reading A13: a channel with w_i = 0 has been REMOVED ("bad channels were
+ * removed before processing"): its samples are never read, so whatever
+ * a flagged channel holds (NaN-blanked planes included) cannot reach F. */
 void oracle_naive(const float *Q, const float *U, long long n_pix,
                   const double *lam2, const double *w, int n_chan,
                   double K, double lambda0_sq,
@@ -96,6 +99,7 @@ void oracle_naive(const float *Q, const float *U, long long n_pix,
         for (int k = 0; k < n_phi; ++k) {
             double sq = 0.0, su = 0.0;
             for (int i = 0; i < n_chan; ++i) {
+                if (w[i] == 0.0) continue; /* A13 */
                 double th = 2.0 * phi[k] * (lam2[i] - lambda0_sq);
                 double c = cos(th), s = sin(th);
                 double q = (double)Q[p * n_chan + i], u = (double)U[p * n_chan + i];
@@ -144,6 +148,7 @@ int oracle_table(const float *Q, const float *U, long long n_pix,
                 const double *c = C + (size_t)k * n_chan, *s = S + (size_t)k * n_chan;
                 double sq = 0.0, su = 0.0;
                 for (int i = 0; i < n_chan; ++i) {
+                    if (w[i] == 0.0) continue; /* A13 */
                     double qi = (double)q[i], ui = (double)u[i];
                     sq += w[i] * (qi * c[i] + ui * s[i]);
                     su += w[i] * (ui * c[i] - qi * s[i]);
@@ -167,6 +172,7 @@ void oracle_tolerance_scale(const float *Q, const float *U, long long n_pix,
     for (long long p = 0; p < n_pix; ++p) {
         double s = 0.0;
         for (int i = 0; i < n_chan; ++i) {
+            if (w[i] == 0.0) continue; /* A13 */
             double q = (double)Q[p * n_chan + i], u = (double)U[p * n_chan + i];
             s += w[i] * sqrt(q * q + u * u);
         }
@@ -192,6 +198,8 @@ static double wrap_half_pi(double a)
  *   edges or when the parabola is not strictly concave;
  *   pa_lambda0 = 0.5 atan2(FU_{k*}, FQ_{k*});
  *   pa_zero    = wrap(pa_lambda0 - phi_peak * lambda_0^2) to [-pi/2, pi/2).
+ * Reading A17: a line of sight with a non-finite |F| at any depth has no peak:
+ *   k* = -1 and NaN in every map.
  */
 void oracle_peaks(const double *FQ, const double *FU, long long n_pix,
                   const double *phi, int n_phi, double lambda0_sq,
@@ -200,11 +208,20 @@ void oracle_peaks(const double *FQ, const double *FU, long long n_pix,
 {
     for (long long p = 0; p < n_pix; ++p) {
         const double *fq = FQ + p * n_phi, *fu = FU + p * n_phi;
-        int kb = 0;
+        int kb = 0, finite = 1;
         double yb = -1.0;
         for (int k = 0; k < n_phi; ++k) {
             double y = sqrt(fq[k] * fq[k] + fu[k] * fu[k]);
+            if (!isfinite(y)) finite = 0;
             if (y > yb) { yb = y; kb = k; }
+        }
+        if (!finite) {
+            /* Reading A17: "where |F~(phi)| is maximum" has no
+             * answer when |F| is not a number at some depth; non-finite samples
+             * propagate (rmsynth.h), so the line of sight reports k* = -1 and NaN. */
+            kstar[p] = -1;
+            peak_amp[p] = peak_phi[p] = pa_lambda0[p] = pa_zero[p] = NAN;
+            continue;
         }
         double amp = yb, ph = phi[kb];
         if (kb > 0 && kb < n_phi - 1) {

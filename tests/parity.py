@@ -34,6 +34,15 @@ def check_peaks(oracle, oplan, FQ, FU, T, got, dphi_min, what=""):
     n = y.shape[0]
     rows = np.arange(n)
     kg, ko = got["kstar"].astype(np.int64), ref["kstar"].astype(np.int64)
+    # reading A17: lines of sight with a non-finite |F| report -1 / NaN on both sides and are compared no further
+    dead = ko < 0
+    if dead.any():
+        assert np.array_equal(kg[dead], ko[dead]), f"{what}: non-finite lines of sight must report index -1"
+        for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+            assert np.all(np.isnan(got[k][dead])), f"{what}: {k} must be NaN on a non-finite line of sight"
+        live = ~dead
+        got = {k: v[live] for k, v in got.items()}
+        return check_peaks(oracle, oplan, FQ[live], FU[live], T[live], got, dphi_min, what) if live.any() else 0
     assert kg.min() >= 0 and kg.max() < y.shape[1]
     gap = y[rows, ko] - y[rows, kg]
     bad = (kg != ko) & (gap > 2 * TOL * T)

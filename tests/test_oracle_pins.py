@@ -240,6 +240,39 @@ def test_p11_brute_force_complex_exp(oracle_mod):
     assert np.max(np.abs(T - Tref)) < 1e-14
 
 
+def test_a13_zero_weight_channels_are_removed(oracle_mod):
+    """Reading A13 ("bad channels were removed before processing"): with w_i = 0 channel i is not part of the
+    sums at all.  F, T_p, K and lambda_0^2 must equal those of the SHORTER problem with the flagged channels deleted,
+    whatever the flagged samples hold -- NaN and Inf included.  Catches: 0 * NaN = NaN leaking into F, flagged
+    channels counted in K or in the mean lambda^2."""
+    rng = np.random.default_rng(9)
+    n = 24
+    nu = lofar_like(n, 1.0e9, 1.5e9)
+    w = rng.uniform(0.2, 1.0, n)
+    flagged = np.array([0, 5, 6, 17, 23])
+    w[flagged] = 0.0
+    phi = np.linspace(-200, 200, 11)
+    Q = rng.standard_normal((6, n)).astype(np.float32)
+    U = rng.standard_normal((6, n)).astype(np.float32)
+    Q[0, 5] = np.nan; U[1, 17] = np.inf; Q[2, 0] = -np.inf; Q[3, flagged] = 1e30; U[4, 23] = np.nan
+    keep = np.setdiff1d(np.arange(n), flagged)
+    full = oracle_mod.make_plan(nu, w, phi)
+    short = oracle_mod.make_plan(nu[keep], w[keep], phi)
+    assert full.K == short.K and abs(full.lambda0_sq - short.lambda0_sq) < 1e-15
+    for fn in (oracle_mod.synth_naive, oracle_mod.synth_table):
+        a = fn(full, Q, U)
+        b = fn(short, np.ascontiguousarray(Q[:, keep]), np.ascontiguousarray(U[:, keep]))
+        assert np.all(np.isfinite(a[0])) and np.all(np.isfinite(a[1]))
+        assert np.max(np.abs(a[0] - b[0])) < 1e-14 and np.max(np.abs(a[1] - b[1])) < 1e-14
+    Ta = oracle_mod.tolerance_scale(full, Q, U)
+    Tb = oracle_mod.tolerance_scale(short, np.ascontiguousarray(Q[:, keep]), np.ascontiguousarray(U[:, keep]))
+    assert np.all(np.isfinite(Ta)) and np.max(np.abs(Ta - Tb)) < 1e-14
+    # a non-finite sample in a channel that is NOT flagged still poisons its line of sight (and only that one)
+    Q[5, 3] = np.nan
+    a = oracle_mod.synth_table(full, Q, U)
+    assert np.all(np.isnan(a[0][5])) and np.all(np.isfinite(a[0][:5]))
+
+
 def test_naive_and_table_agree_on_config1_sample(oracle_mod):
     """oracle_table vs oracle_naive to 1e-12 T_p on real config-1 inputs."""
     import torch
@@ -322,6 +355,21 @@ def test_p12_pa_zero_wraps_to_half_open_interval(oracle_mod):
     plan = oracle_mod.make_plan(nu, None, [0.0])
     r = oracle_mod.peaks(plan, np.array([[-1.0], [-1.0]]), np.array([[1e-9], [-1e-9]]))
     assert abs(r["pa_lambda0"][0] - np.pi / 2) < 1e-8 and abs(r["pa_lambda0"][1] + np.pi / 2) < 1e-8
+
+
+def test_p12_nonfinite_line_of_sight_has_no_peak(oracle_mod):
+    """Reading A17: P:L123 defines phi_peak as the depth "where |F~(phi)| is maximum"; with a NaN or Inf in |F|
+    the maximum does not exist.  Non-finite samples propagate (rmsynth.h), so such a line of sight reports
+    k* = -1 and NaN maps, and its finite neighbours are untouched.  Catches: a NaN silently skipped by `>`
+    (the peak of the remaining samples reported as if nothing happened)."""
+    plan = oracle_mod.make_plan(lofar_like(8), None, np.arange(5.0))
+    FQ = np.array([[1.0, 3, 2, 1, 0], [1.0, np.nan, 2, 1, 0], [1.0, 3, 2, np.inf, 0], [0.0, 1, 5, 1, 0]])
+    FU = np.zeros_like(FQ)
+    FU[3, 2] = -np.inf
+    r = oracle_mod.peaks(plan, FQ, FU)
+    assert list(r["kstar"]) == [1, -1, -1, -1]
+    for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+        assert np.isfinite(r[k][0]) and np.all(np.isnan(r[k][1:])), k
 
 
 # ---------------------------------------------------------------- P13: slab generator
