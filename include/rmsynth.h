@@ -67,8 +67,12 @@ typedef struct {
     int struct_size;   /* sizeof(rmsynth_options); lets the struct grow                   */
     int scheme;        /* RMSYNTH_SCHEME_*                                                */
     int lambda0_mode;  /* 0 weighted mean (default), 1 plain mean, 2 explicit lambda0_sq  */
-    int device;        /* CUDA device ordinal, -1 = current device                        */
+    int device;        /* CUDA device ordinal, -1 = the caller's current device.  Every call  */
+                       /* on the plan runs on this device and restores the caller's current   */
+                       /* device before returning; streams passed in must belong to it.       */
     double lambda0_sq; /* used when lambda0_mode == 2 (0 reproduces Fig. 1 left)  */
+    long long host_chunk_pixels; /* pixels per chunk of rmsynth_execute_host / _stream (rounded */
+                       /* to a multiple of 4); 0 = automatic (~256 MB of device buffers per slot) */
 } rmsynth_options;
 
 /* Build a plan: lambda_i^2, K, lambda_0^2 on the host in FP64 ("computed only once"),
@@ -136,13 +140,35 @@ rmsynth_status rmsynth_execute_ex(const rmsynth_plan *plan, const float *Q, cons
                                   void *stream);
 
 /* Same as rmsynth_execute_peaks with every cube/map pointer in HOST memory (pinned memory
- * gives full PCIe rate): the library streams pixel chunks host->device->host through its own
- * device buffers, overlapping copies with compute, and returns when the outputs are complete.
- * Each datum crosses the bus once (the paper's transfer rule).  Synchronous. */
+ * gives full PCIe rate): the library streams pixel chunks host->device->host through three
+ * sets of device buffers, with H2D of chunk i+1, the kernels of chunk i and D2H of chunk i-1
+ * overlapping, and returns when the outputs are complete.  Chunk size: the plan's
+ * host_chunk_pixels.  Each datum crosses the bus once (the paper's transfer rule,
+ * P:L200-210).  Synchronous. */
 rmsynth_status rmsynth_execute_host(const rmsynth_plan *plan, const float *Q, const float *U,
                                     long long n_pix, int layout, float *FQ, float *FU,
                                     float *peak_amp, float *peak_phi, float *pa_lambda0,
                                     float *pa_zero, int *peak_index);
+
+/* Out-of-core form of rmsynth_execute_host for cubes that do not fit in host memory (the paper's LOFAR_HR
+ * shape is 110 GB in and > 1 TB out): the library owns three sets of pinned staging buffers and
+ * calls back on the caller's thread, in chunk order,
+ *   n = fill(user, i, Q, U, max_pix)   write chunk i (n <= max_pix lines of sight, n = 0 ends the run) into
+ *                                      the HOST staging buffers Q, U: compact, input layout per `layout`,
+ *                                      i.e. Q[c*n + p] (IN_FREQ_MAJOR) or Q[p*n_chan + c] (IN_LOS_MAJOR)
+ *   drain(user, i, n, out)             chunk i is complete: out->FQ/FU (compact [k*n + p] or [p*n_phi + k],
+ *                                      if RMSYNTH_WANT_CUBES) and out->peak_* (if RMSYNTH_WANT_MAPS) point
+ *                                      into HOST staging that is valid only during the call
+ * while chunks i+1, i+2 are in flight (H2D, kernels and D2H overlap; each datum crosses the bus once,
+ * P:L200-210).  max_pix is the plan's host_chunk_pixels (or the automatic size).  *n_pix_done (may be
+ * NULL) receives the number of lines of sight processed.  Synchronous; EINVAL on NULL callbacks, unknown
+ * flags, or a fill() that returns more than max_pix. */
+enum { RMSYNTH_WANT_CUBES = 1, RMSYNTH_WANT_MAPS = 2 };
+typedef long long (*rmsynth_fill_fn)(void *user, long long chunk_index, float *Q, float *U, long long max_pix);
+typedef void (*rmsynth_drain_fn)(void *user, long long chunk_index, long long n_pix, const rmsynth_outputs *out);
+rmsynth_status rmsynth_execute_stream(const rmsynth_plan *plan, int layout, int outputs,
+                                      rmsynth_fill_fn fill, rmsynth_drain_fn drain, void *user,
+                                      long long *n_pix_done);
 
 /* R(phi) of Eq. 12 in FP64.  phi_eval HOST [n] or NULL for the plan grid (then n must be
  * n_phi); R_re, R_im HOST [n].  Synchronous. */

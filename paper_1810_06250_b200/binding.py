@@ -26,13 +26,14 @@ IN_LOS_MAJOR, IN_FREQ_MAJOR, OUT_LOS_MAJOR, OUT_PHI_MAJOR = 0, 1, 0, 2
 SCHEME_AUTO, SCHEME_TF32X3, SCHEME_F16X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS = 0, 1, 2, 3, 4
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
-           "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_rmsf",
+           "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_execute_stream",
+           "rmsynth_rmsf",
            "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
 
 
 class Options(C.Structure):
     _fields_ = [("struct_size", C.c_int), ("scheme", C.c_int), ("lambda0_mode", C.c_int),
-                ("device", C.c_int), ("lambda0_sq", C.c_double)]
+                ("device", C.c_int), ("lambda0_sq", C.c_double), ("host_chunk_pixels", C.c_longlong)]
 
 
 class Outputs(C.Structure):
@@ -50,6 +51,10 @@ _lib.rmsynth_execute.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp,
 _lib.rmsynth_execute_peaks.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
 _lib.rmsynth_execute_ex.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, C.POINTER(Outputs), _vp]
 _lib.rmsynth_execute_host.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _fp, _fp, _ip]
+FILL_FN = C.CFUNCTYPE(C.c_longlong, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p, C.c_longlong)
+DRAIN_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_longlong, C.c_longlong, C.POINTER(Outputs))
+WANT_CUBES, WANT_MAPS = 1, 2
+_lib.rmsynth_execute_stream.argtypes = [_vp, C.c_int, C.c_int, FILL_FN, DRAIN_FN, C.c_void_p, C.POINTER(C.c_longlong)]
 _lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
 _lib.rmsynth_launch_count.argtypes = [C.c_int]
 _lib.rmsynth_launch_count.restype = C.c_longlong
@@ -100,13 +105,13 @@ def rmsynth_launch_count(reset: bool = False) -> int:
 class Plan:
     """Owns an rmsynth_plan*.  Methods carry the C entry-point names without the prefix."""
 
-    def __init__(self, nu_hz, w, phi, scheme=SCHEME_AUTO, lambda0_mode=0, lambda0_sq=0.0, device=-1):
+    def __init__(self, nu_hz, w, phi, scheme=SCHEME_AUTO, lambda0_mode=0, lambda0_sq=0.0, device=-1, host_chunk_pixels=0):
         nu = np.ascontiguousarray(nu_hz, dtype=np.float64)
         ph = np.ascontiguousarray(phi, dtype=np.float64)
         ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
         if ww is not None and ww.size != nu.size:
             raise ValueError("w and nu_hz differ in length")
-        opt = Options(C.sizeof(Options), scheme, lambda0_mode, device, lambda0_sq)
+        opt = Options(C.sizeof(Options), scheme, lambda0_mode, device, lambda0_sq, host_chunk_pixels)
         self._h = _vp()
         _check(_lib.rmsynth_plan_create(C.byref(self._h), _d(nu), _d(ww), nu.size, _d(ph), ph.size, C.byref(opt)))
         K, l0 = C.c_double(), C.c_double()
@@ -157,3 +162,34 @@ class Plan:
         _check(_lib.rmsynth_execute_host(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
                                          _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
                                          _ptr(peak_index)))
+
+    def execute_stream(self, layout, outputs, fill, drain):
+        """fill(i, Q, U, max_pix) -> n and drain(i, n, out) are Python callables; Q, U are numpy views of the
+        library's pinned staging buffers (flat, max_pix * n_chan floats each), out is a dict of numpy views that are
+        valid only during the call.  Returns the number of lines of sight processed."""
+        nc, npz = self.n_chan, self.n_phi
+
+        def _fill(_, i, q, u, max_pix):
+            qa = np.ctypeslib.as_array(C.cast(q, C.POINTER(C.c_float)), shape=(max_pix * nc,))
+            ua = np.ctypeslib.as_array(C.cast(u, C.POINTER(C.c_float)), shape=(max_pix * nc,))
+            return int(fill(i, qa, ua, max_pix))
+
+        def _drain(_, i, n, out):
+            o = out.contents
+            view = {}
+            for name in ("FQ", "FU"):
+                a = getattr(o, name)
+                if a:
+                    view[name] = np.ctypeslib.as_array(C.cast(a, C.POINTER(C.c_float)), shape=(n * npz,))
+            for name in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+                a = getattr(o, name)
+                if a:
+                    view[name] = np.ctypeslib.as_array(C.cast(a, C.POINTER(C.c_float)), shape=(n,))
+            if o.peak_index:
+                view["peak_index"] = np.ctypeslib.as_array(C.cast(o.peak_index, C.POINTER(C.c_int)), shape=(n,))
+            drain(i, n, view)
+
+        done = C.c_longlong(0)
+        cb_fill, cb_drain = FILL_FN(_fill), DRAIN_FN(_drain)
+        _check(_lib.rmsynth_execute_stream(self._h, layout, outputs, cb_fill, cb_drain, None, C.byref(done)))
+        return done.value

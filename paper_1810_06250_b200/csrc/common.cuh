@@ -31,6 +31,24 @@ inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_
             return rms::fail(RMSYNTH_ECUDA, std::string(name) + " launch: " + cudaGetErrorString(e__)); \
     } while (0)
 
+// Every entry point that touches the device runs on the PLAN's device whatever the caller's current device is, and
+// leaves the caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && dev >= 0 && prev != dev) {
+            err = cudaSetDevice(dev);
+            switched = err == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
 // Tensor-path operand geometry chosen at plan time (see tc_gemm.cu).
 struct TcGeom {
     int n_tile = 0;      // phi columns per tile (n); UMMA N = 2n
@@ -66,19 +84,20 @@ struct rmsynth_plan {
     // FP16 split tensor path (tc_gemm3.cu)
     rms::TcGeom tc3;
     void* d_tcB3 = nullptr;               // scaled FP16 hi/lo B operand blobs
-    unsigned int* d_tc3mask = nullptr;    // per 32-channel chunk: channels with w > 0
+    unsigned int* d_chanmask = nullptr;   // per 32 channels: bit i set = channel exists and has w > 0 (reading A13)
     int tc3_eb = 0;                       // B is scaled by 2^tc3_eb
     void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
-    static constexpr int kScratch = 10;   // 0-7 host-stream slots (Q,U,FQ,FU x2); 8,9 their maps
+    static constexpr int kScratch = 15;   // host-streaming slots: (Q, U, FQ, FU, maps) x 3
     mutable float* scratch[kScratch] = {};
     mutable size_t scratch_bytes[kScratch] = {};
     // per-call workspace keyed by (stream, tag) so that concurrent calls on different streams never share it
     struct StreamScratch { cudaStream_t st; int tag; float* ptr; size_t bytes; };
     mutable std::mutex pool_mu;
     mutable std::vector<StreamScratch> pool;
-    mutable cudaStream_t hs[2] = {nullptr, nullptr};
+    mutable void* host_pipe = nullptr;    // streams, events and staging of the host-streaming engine (execute.cu)
+    long long host_chunk_pixels = 0;      // rmsynth_options.host_chunk_pixels (0 = automatic)
 };
 
 namespace rms {
@@ -92,6 +111,8 @@ rmsynth_status fp32_table_execute(const rmsynth_plan* p, const float* Q, const f
                                   int layout, float* FQ, float* FU, cudaStream_t st);
 rmsynth_status fp32_sincos_execute(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix,
                                    int layout, float* FQ, float* FU, cudaStream_t st);
+// execute.cu
+void host_pipe_free(rmsynth_plan* p);
 // peaks.cu
 rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,
                              float* pa0, float* paz, int* idx, cudaStream_t st);

@@ -1,6 +1,8 @@
-// rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_ex / rmsynth_execute_host: argument checks,
-// scheme dispatch (rows a4-a9) and the host-streaming loop (the paper's "each datum crosses the bus
-// once" rule, with pixel chunks instead of LOS batches sized from GPU memory P:L210).
+// rmsynth_execute / rmsynth_execute_peaks / rmsynth_execute_ex: argument checks and scheme dispatch (rows a4-a9);
+// rmsynth_execute_host / rmsynth_execute_stream: the out-of-core host-streaming engine (scope row NEXT-2) -- the paper's
+// "a given piece of data is moved between the CPU and the GPU only once" rule with pixel chunks instead of
+// LOS batches sized from GPU memory: three device slots, one stream per direction and one for the kernels, so
+// that H2D(i+1), compute(i) and D2H(i-1) overlap.
 #include <cstdlib>
 #include <cstring>
 #include "common.cuh"
@@ -32,6 +34,8 @@ static rmsynth_status check_args(const rmsynth_plan* p, const float* Q, const fl
 // Device-resident contraction + optional |F| cube and maps on one stream; never synchronises.
 static rmsynth_status run_device(const rmsynth_plan* p, const float* Q, const float* U, long long n_pix, int layout,
                                  Outs o, cudaStream_t st) {
+    DeviceGuard g(p->device);
+    RMS_CUDA(g.err);
     if (p->scheme == RMSYNTH_SCHEME_TF32X3 || p->scheme == RMSYNTH_SCHEME_F16X3)
         return tc_execute(p, Q, U, n_pix, layout, o.FQ, o.FU, o.FA, o.amp, o.phi, o.pa0, o.paz, o.idx, st);
     // FP32 CUDA-core comparison paths: cubes first, then the stand-alone |F| and peak kernels.
@@ -46,6 +50,136 @@ static rmsynth_status run_device(const rmsynth_plan* p, const float* Q, const fl
     if (s == RMSYNTH_OK && o.FA) s = abs_from_cubes(o.FQ, o.FU, n_pix * p->n_phi, o.FA, st);
     if (s != RMSYNTH_OK || !o.maps()) return s;
     return peaks_from_cubes(p, o.FQ, o.FU, n_pix, layout & RMSYNTH_OUT_PHI_MAJOR, o.amp, o.phi, o.pa0, o.paz, o.idx, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host streaming engine.  Slot b holds one pixel chunk: inputs dQ,dU [chunk x n_chan], cubes dFQ,dFU [chunk x n_phi]
+// (only if cubes are wanted) and five maps.  Per chunk i in slot b = i % 3:
+//   s_in : wait run_done[b] (the chunk that last used these input buffers has been computed) -> H2D -> in_done[b]
+//   s_run: wait in_done[b], out_done[b] (the slot's previous outputs have left)               -> kernels -> run_done[b]
+//   s_out: wait run_done[b]                                                                   -> D2H -> out_done[b]
+constexpr int kSlots = 3;
+
+struct HostPipe {
+    cudaStream_t s_in = nullptr, s_run = nullptr, s_out = nullptr;
+    cudaEvent_t in_done[kSlots] = {}, run_done[kSlots] = {}, out_done[kSlots] = {};
+    float *dQ[kSlots] = {}, *dU[kSlots] = {}, *dFQ[kSlots] = {}, *dFU[kSlots] = {}, *dM[kSlots] = {};
+    float* hIn[kSlots] = {};    // pinned staging of rmsynth_execute_stream: Q then U
+    float* hOut[kSlots] = {};   //                                             FQ, FU, then five maps
+    size_t in_bytes = 0, out_bytes = 0;
+};
+
+static rmsynth_status pipe_get(const rmsynth_plan* p, HostPipe** out) {
+    if (!p->host_pipe) {
+        HostPipe* hp = new HostPipe;
+        p->host_pipe = hp;
+        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_in, cudaStreamNonBlocking));
+        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_run, cudaStreamNonBlocking));
+        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_out, cudaStreamNonBlocking));
+        for (int b = 0; b < kSlots; ++b) {
+            RMS_CUDA(cudaEventCreateWithFlags(&hp->in_done[b], cudaEventDisableTiming));
+            RMS_CUDA(cudaEventCreateWithFlags(&hp->run_done[b], cudaEventDisableTiming));
+            RMS_CUDA(cudaEventCreateWithFlags(&hp->out_done[b], cudaEventDisableTiming));
+        }
+    }
+    *out = static_cast<HostPipe*>(p->host_pipe);
+    return RMSYNTH_OK;
+}
+
+void host_pipe_free(rmsynth_plan* p) {
+    HostPipe* hp = static_cast<HostPipe*>(p->host_pipe);
+    if (!hp) return;
+    for (int b = 0; b < kSlots; ++b) {
+        if (hp->in_done[b]) cudaEventDestroy(hp->in_done[b]);
+        if (hp->run_done[b]) cudaEventDestroy(hp->run_done[b]);
+        if (hp->out_done[b]) cudaEventDestroy(hp->out_done[b]);
+        if (hp->hIn[b]) cudaFreeHost(hp->hIn[b]);
+        if (hp->hOut[b]) cudaFreeHost(hp->hOut[b]);
+    }
+    if (hp->s_in) cudaStreamDestroy(hp->s_in);
+    if (hp->s_run) cudaStreamDestroy(hp->s_run);
+    if (hp->s_out) cudaStreamDestroy(hp->s_out);
+    delete hp;
+    p->host_pipe = nullptr;
+}
+
+// pixels per chunk: the plan option, else ~256 MB of device buffers per slot; a multiple of 4 (the FP16 kernel's
+// fast paths want 16-byte rows), at least 4, at most n_pix
+static long long chunk_pixels(const rmsynth_plan* p, long long n_pix, bool cubes) {
+    long long chunk = p->host_chunk_pixels;
+    if (chunk <= 0) {
+        chunk = (256LL << 20) / (8LL * (p->n_chan + (cubes ? p->n_phi : 0)));
+        chunk = chunk / 1024 * 1024;
+        if (chunk < 1024) chunk = 1024;
+    }
+    chunk = (chunk + 3) & ~3LL;
+    if (n_pix > 0 && chunk > n_pix) chunk = n_pix;
+    return chunk;
+}
+
+static rmsynth_status pipe_buffers(const rmsynth_plan* p, HostPipe* hp, long long chunk, bool cubes) {
+    rmsynth_status s;
+    for (int b = 0; b < kSlots; ++b)
+        if ((s = ensure_scratch(p, 5 * b + 0, sizeof(float) * chunk * p->n_chan, &hp->dQ[b])) ||
+            (s = ensure_scratch(p, 5 * b + 1, sizeof(float) * chunk * p->n_chan, &hp->dU[b])) ||
+            (s = ensure_scratch(p, 5 * b + 2, cubes ? sizeof(float) * chunk * p->n_phi : 0, &hp->dFQ[b])) ||   // maps only: no cube buffers
+            (s = ensure_scratch(p, 5 * b + 3, cubes ? sizeof(float) * chunk * p->n_phi : 0, &hp->dFU[b])) ||
+            (s = ensure_scratch(p, 5 * b + 4, sizeof(float) * chunk * 5, &hp->dM[b])))
+            return s;
+    return RMSYNTH_OK;
+}
+
+// One chunk through slot b.  hQ/hU point at the chunk's first pixel in HOST memory; for frequency-major input in_pitch is
+// the host row pitch in pixels (n_pix of the whole cube, or the chunk's own pixel count for compact staging buffers);
+// likewise out_pitch for phi-major cubes.  Maps go to ho.amp.. (already offset to the chunk's first pixel).
+static rmsynth_status pipe_chunk(const rmsynth_plan* p, HostPipe* hp, int b, long long chunk, long long n, int layout,
+                                 const float* hQ, const float* hU, long long in_pitch, const Outs& ho, long long out_pitch) {
+    const int nc = p->n_chan, np = p->n_phi;
+    const bool in_freq = layout & RMSYNTH_IN_FREQ_MAJOR, out_phi = layout & RMSYNTH_OUT_PHI_MAJOR;
+    RMS_CUDA(cudaStreamWaitEvent(hp->s_in, hp->run_done[b], 0));
+    if (in_freq) {   // columns of [chan][pitch] -> compact [chan][n]
+        RMS_CUDA(cudaMemcpy2DAsync(hp->dQ[b], n * 4, hQ, in_pitch * 4, n * 4, nc, cudaMemcpyHostToDevice, hp->s_in));
+        RMS_CUDA(cudaMemcpy2DAsync(hp->dU[b], n * 4, hU, in_pitch * 4, n * 4, nc, cudaMemcpyHostToDevice, hp->s_in));
+    } else {
+        RMS_CUDA(cudaMemcpyAsync(hp->dQ[b], hQ, sizeof(float) * n * nc, cudaMemcpyHostToDevice, hp->s_in));
+        RMS_CUDA(cudaMemcpyAsync(hp->dU[b], hU, sizeof(float) * n * nc, cudaMemcpyHostToDevice, hp->s_in));
+    }
+    RMS_CUDA(cudaEventRecord(hp->in_done[b], hp->s_in));
+    RMS_CUDA(cudaStreamWaitEvent(hp->s_run, hp->in_done[b], 0));
+    RMS_CUDA(cudaStreamWaitEvent(hp->s_run, hp->out_done[b], 0));
+    float* m = hp->dM[b];
+    Outs o;
+    if (ho.FQ) { o.FQ = hp->dFQ[b]; o.FU = hp->dFU[b]; }
+    o.amp = ho.amp ? m : nullptr;
+    o.phi = ho.phi ? m + chunk : nullptr;
+    o.pa0 = ho.pa0 ? m + 2 * chunk : nullptr;
+    o.paz = ho.paz ? m + 3 * chunk : nullptr;
+    o.idx = ho.idx ? (int*)(m + 4 * chunk) : nullptr;
+    rmsynth_status s = run_device(p, hp->dQ[b], hp->dU[b], n, layout, o, hp->s_run);
+    if (s != RMSYNTH_OK) return s;
+    RMS_CUDA(cudaEventRecord(hp->run_done[b], hp->s_run));
+    RMS_CUDA(cudaStreamWaitEvent(hp->s_out, hp->run_done[b], 0));
+    if (ho.FQ) {
+        if (out_phi) {
+            RMS_CUDA(cudaMemcpy2DAsync(ho.FQ, out_pitch * 4, hp->dFQ[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, hp->s_out));
+            RMS_CUDA(cudaMemcpy2DAsync(ho.FU, out_pitch * 4, hp->dFU[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, hp->s_out));
+        } else {
+            RMS_CUDA(cudaMemcpyAsync(ho.FQ, hp->dFQ[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, hp->s_out));
+            RMS_CUDA(cudaMemcpyAsync(ho.FU, hp->dFU[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, hp->s_out));
+        }
+    }
+    float* outs[5] = {ho.amp, ho.phi, ho.pa0, ho.paz, (float*)ho.idx};
+    for (int j = 0; j < 5; ++j)
+        if (outs[j]) RMS_CUDA(cudaMemcpyAsync(outs[j], m + j * chunk, sizeof(float) * n, cudaMemcpyDeviceToHost, hp->s_out));
+    RMS_CUDA(cudaEventRecord(hp->out_done[b], hp->s_out));
+    return RMSYNTH_OK;
+}
+
+static rmsynth_status pipe_drain(HostPipe* hp) {
+    RMS_CUDA(cudaStreamSynchronize(hp->s_in));
+    RMS_CUDA(cudaStreamSynchronize(hp->s_run));
+    RMS_CUDA(cudaStreamSynchronize(hp->s_out));
+    return RMSYNTH_OK;
 }
 
 }  // namespace rms
@@ -93,65 +227,106 @@ rmsynth_status rmsynth_execute_host(const rmsynth_plan* plan, const float* Q, co
     rmsynth_status s = check_args(plan, Q, U, n_pix, layout, false, ho);
     if (s != RMSYNTH_OK || n_pix == 0) return s;
     const rmsynth_plan* p = plan;
-    RMS_CUDA(cudaSetDevice(p->device));
-    std::lock_guard<std::mutex> g(p->mu);
+    DeviceGuard g(p->device);
+    RMS_CUDA(g.err);
+    std::lock_guard<std::mutex> lock(p->mu);
     const int nc = p->n_chan, np = p->n_phi;
     const bool in_freq = layout & RMSYNTH_IN_FREQ_MAJOR, out_phi = layout & RMSYNTH_OUT_PHI_MAJOR;
-    // ~256 MB of device buffers per slot, two slots in flight
-    static const long long chunk_mb = getenv("RMSYNTH_HOST_CHUNK_MB") ? atoll(getenv("RMSYNTH_HOST_CHUNK_MB")) : 256;
-    long long chunk = ((chunk_mb > 0 ? chunk_mb : 256) << 20) / (8LL * (nc + np));
-    chunk = chunk / 1024 * 1024;
-    if (chunk < 1024) chunk = 1024;
-    if (chunk > n_pix) chunk = n_pix;
-    float *dQ[2], *dU[2], *dFQ[2], *dFU[2], *dM[2];
-    for (int b = 0; b < 2; ++b) {
-        if (!p->hs[b]) RMS_CUDA(cudaStreamCreateWithFlags(&p->hs[b], cudaStreamNonBlocking));
-        if ((s = ensure_scratch(p, 4 * b + 0, sizeof(float) * chunk * nc, &dQ[b])) ||
-            (s = ensure_scratch(p, 4 * b + 1, sizeof(float) * chunk * nc, &dU[b])) ||
-            (s = ensure_scratch(p, 4 * b + 2, FQ ? sizeof(float) * chunk * np : 0, &dFQ[b])) ||    // maps only: no cube buffers
-            (s = ensure_scratch(p, 4 * b + 3, FQ ? sizeof(float) * chunk * np : 0, &dFU[b])) ||
-            (s = ensure_scratch(p, 8 + b, sizeof(float) * chunk * 5, &dM[b])))
-            return s;
-    }
+    const long long chunk = chunk_pixels(p, n_pix, FQ != nullptr);
+    HostPipe* hp;
+    if ((s = pipe_get(p, &hp)) || (s = pipe_buffers(p, hp, chunk, FQ != nullptr))) return s;
     int it = 0;
     for (long long p0 = 0; p0 < n_pix; p0 += chunk, ++it) {
-        const int b = it & 1;
         const long long n = n_pix - p0 < chunk ? n_pix - p0 : chunk;
-        cudaStream_t st = p->hs[b];
-        if (in_freq) {   // columns [p0, p0+n) of [chan][pix] -> compact [chan][n]
-            RMS_CUDA(cudaMemcpy2DAsync(dQ[b], n * 4, Q + p0, n_pix * 4, n * 4, nc, cudaMemcpyHostToDevice, st));
-            RMS_CUDA(cudaMemcpy2DAsync(dU[b], n * 4, U + p0, n_pix * 4, n * 4, nc, cudaMemcpyHostToDevice, st));
-        } else {
-            RMS_CUDA(cudaMemcpyAsync(dQ[b], Q + p0 * nc, sizeof(float) * n * nc, cudaMemcpyHostToDevice, st));
-            RMS_CUDA(cudaMemcpyAsync(dU[b], U + p0 * nc, sizeof(float) * n * nc, cudaMemcpyHostToDevice, st));
-        }
-        float* m = dM[b];
         Outs o;
-        if (FQ) { o.FQ = dFQ[b]; o.FU = dFU[b]; }
-        o.amp = peak_amp ? m : nullptr;
-        o.phi = peak_phi ? m + chunk : nullptr;
-        o.pa0 = pa_lambda0 ? m + 2 * chunk : nullptr;
-        o.paz = pa_zero ? m + 3 * chunk : nullptr;
-        o.idx = peak_index ? (int*)(m + 4 * chunk) : nullptr;
-        s = run_device(p, dQ[b], dU[b], n, layout, o, st);
-        if (s != RMSYNTH_OK) return s;
         if (FQ) {
-            if (out_phi) {
-                RMS_CUDA(cudaMemcpy2DAsync(FQ + p0, n_pix * 4, dFQ[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, st));
-                RMS_CUDA(cudaMemcpy2DAsync(FU + p0, n_pix * 4, dFU[b], n * 4, n * 4, np, cudaMemcpyDeviceToHost, st));
-            } else {
-                RMS_CUDA(cudaMemcpyAsync(FQ + p0 * np, dFQ[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, st));
-                RMS_CUDA(cudaMemcpyAsync(FU + p0 * np, dFU[b], sizeof(float) * n * np, cudaMemcpyDeviceToHost, st));
-            }
+            o.FQ = out_phi ? FQ + p0 : FQ + p0 * np;
+            o.FU = out_phi ? FU + p0 : FU + p0 * np;
         }
-        float* outs[5] = {peak_amp, peak_phi, pa_lambda0, pa_zero, (float*)peak_index};
-        for (int j = 0; j < 5; ++j)
-            if (outs[j])
-                RMS_CUDA(cudaMemcpyAsync(outs[j] + p0, m + j * chunk, sizeof(float) * n, cudaMemcpyDeviceToHost, st));
+        o.amp = peak_amp ? peak_amp + p0 : nullptr;
+        o.phi = peak_phi ? peak_phi + p0 : nullptr;
+        o.pa0 = pa_lambda0 ? pa_lambda0 + p0 : nullptr;
+        o.paz = pa_zero ? pa_zero + p0 : nullptr;
+        o.idx = peak_index ? peak_index + p0 : nullptr;
+        s = pipe_chunk(p, hp, it % kSlots, chunk, n, layout, in_freq ? Q + p0 : Q + p0 * nc, in_freq ? U + p0 : U + p0 * nc, n_pix, o, n_pix);
+        if (s != RMSYNTH_OK) {
+            pipe_drain(hp);
+            return s;
+        }
     }
-    RMS_CUDA(cudaStreamSynchronize(p->hs[0]));
-    RMS_CUDA(cudaStreamSynchronize(p->hs[1]));
-    return RMSYNTH_OK;
+    return pipe_drain(hp);
+}
+
+rmsynth_status rmsynth_execute_stream(const rmsynth_plan* plan, int layout, int outputs, rmsynth_fill_fn fill,
+                                      rmsynth_drain_fn drain, void* user, long long* n_pix_done) {
+    if (n_pix_done) *n_pix_done = 0;
+    if (!plan) return fail(RMSYNTH_EINVAL, "plan is NULL");
+    if (layout & ~3) return fail(RMSYNTH_EINVAL, "unknown layout flags");
+    if (!fill || !drain) return fail(RMSYNTH_EINVAL, "fill/drain callback is NULL");
+    if (!(outputs & (RMSYNTH_WANT_CUBES | RMSYNTH_WANT_MAPS)) || (outputs & ~(RMSYNTH_WANT_CUBES | RMSYNTH_WANT_MAPS)))
+        return fail(RMSYNTH_EINVAL, "outputs must be RMSYNTH_WANT_CUBES and/or RMSYNTH_WANT_MAPS");
+    const rmsynth_plan* p = plan;
+    DeviceGuard g(p->device);
+    RMS_CUDA(g.err);
+    std::lock_guard<std::mutex> lock(p->mu);
+    const int nc = p->n_chan, np = p->n_phi;
+    const bool cubes = outputs & RMSYNTH_WANT_CUBES, maps = outputs & RMSYNTH_WANT_MAPS;
+    const long long chunk = chunk_pixels(p, 0, cubes);
+    rmsynth_status s;
+    HostPipe* hp;
+    if ((s = pipe_get(p, &hp)) || (s = pipe_buffers(p, hp, chunk, cubes))) return s;
+    const size_t in_bytes = sizeof(float) * 2 * (size_t)chunk * nc;
+    const size_t out_bytes = sizeof(float) * (size_t)chunk * ((cubes ? 2 * (size_t)np : 0) + 5);
+    if (hp->in_bytes < in_bytes || hp->out_bytes < out_bytes) {
+        for (int b = 0; b < kSlots; ++b) {
+            if (hp->hIn[b]) cudaFreeHost(hp->hIn[b]);
+            if (hp->hOut[b]) cudaFreeHost(hp->hOut[b]);
+            hp->hIn[b] = hp->hOut[b] = nullptr;
+        }
+        hp->in_bytes = hp->out_bytes = 0;
+        for (int b = 0; b < kSlots; ++b) {
+            RMS_CUDA(cudaMallocHost(&hp->hIn[b], in_bytes));
+            RMS_CUDA(cudaMallocHost(&hp->hOut[b], out_bytes));
+        }
+        hp->in_bytes = in_bytes;
+        hp->out_bytes = out_bytes;
+    }
+    long long count[kSlots] = {0, 0, 0}, total = 0;
+    auto finish = [&](long long i) -> rmsynth_status {       // chunk i's outputs are in host staging: hand them over
+        const int b = (int)(i % kSlots);
+        RMS_CUDA(cudaEventSynchronize(hp->out_done[b]));
+        const long long n = count[b];
+        float* o = hp->hOut[b];
+        rmsynth_outputs ro;
+        std::memset(&ro, 0, sizeof(ro));
+        ro.struct_size = (int)sizeof(ro);
+        if (cubes) { ro.FQ = o; ro.FU = o + (size_t)n * np; o += 2 * (size_t)n * np; }
+        if (maps) { ro.peak_amp = o; ro.peak_phi = o + n; ro.pa_lambda0 = o + 2 * n; ro.pa_zero = o + 3 * n; ro.peak_index = (int*)(o + 4 * n); }
+        drain(user, i, n, &ro);
+        total += n;
+        return RMSYNTH_OK;
+    };
+    long long i = 0;
+    for (;; ++i) {
+        const int b = (int)(i % kSlots);
+        if (i >= kSlots && (s = finish(i - kSlots))) break;   // frees slot b's staging buffers
+        float* hq = hp->hIn[b];
+        const long long n = fill(user, i, hq, hq + (size_t)chunk * nc, chunk);
+        if (n <= 0) break;
+        if (n > chunk) { s = fail(RMSYNTH_EINVAL, "fill callback returned more pixels than the chunk holds"); break; }
+        count[b] = n;
+        // staging is compact: [chan][n] / [n][chan] with U starting at Q + chunk*n_chan; outputs [phi][n] / [n][phi]
+        float* o = hp->hOut[b];
+        Outs ho;
+        if (cubes) { ho.FQ = o; ho.FU = o + (size_t)n * np; o += 2 * (size_t)n * np; }
+        if (maps) { ho.amp = o; ho.phi = o + n; ho.pa0 = o + 2 * n; ho.paz = o + 3 * n; ho.idx = (int*)(o + 4 * n); }
+        if ((s = pipe_chunk(p, hp, b, chunk, n, layout, hq, hq + (size_t)chunk * nc, n, ho, n))) break;
+    }
+    // chunks 0 .. i-1 were submitted; the loop has handed over all but the last kSlots - 1 of them
+    for (long long j = i > kSlots - 1 ? i - (kSlots - 1) : 0; j < i && s == RMSYNTH_OK; ++j) s = finish(j);
+    pipe_drain(hp);
+    if (n_pix_done) *n_pix_done = total;
+    return s;
 }
 
 }  // extern "C"

@@ -18,7 +18,7 @@ constexpr int TK = 16;   // channels per step
 template <int IN, int OUT>
 __global__ void __launch_bounds__(256) fp32_table_kernel(
     const float* __restrict__ Q, const float* __restrict__ U, long long n_pix, int n_chan, int n_phi,
-    const float* __restrict__ Bc, const float* __restrict__ Bs, int ldb,
+    const float* __restrict__ Bc, const float* __restrict__ Bs, int ldb, const float* __restrict__ kwf,
     float* __restrict__ FQ, float* __restrict__ FU) {
     __shared__ float sQ[TK][TM + 4], sU[TK][TM + 4], sC[TK][TN + 4], sS[TK][TN + 4];
     const int tid = threadIdx.x;
@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(256) fp32_table_kernel(
             long long p = p0 + m;
             int ch = c0 + c;
             float q = 0.f, u = 0.f;
-            if (p < n_pix && ch < n_chan) {
+            if (p < n_pix && ch < n_chan && kwf[ch] != 0.f) {   // reading A13: zero-weight channels are never read
                 size_t off = IN == 0 ? (size_t)p * n_chan + ch : (size_t)ch * n_pix + p;
                 q = Q[off];
                 u = U[off];
@@ -119,7 +119,7 @@ rmsynth_status fp32_table_execute(const rmsynth_plan* p, const float* Q, const f
     const int in = layout & 1, out = (layout >> 1) & 1;
 #define RMS_GO(I, O)                                                                                       \
     fp32_table_kernel<I, O><<<grid, 256, 0, st>>>(Q, U, n_pix, p->n_chan, p->n_phi, p->d_cos, p->d_sin, \
-                                                    p->ldb, FQ, FU)
+                                                    p->ldb, p->d_kwf, FQ, FU)
     if (in == 0 && out == 0) RMS_GO(0, 0);
     else if (in == 0) RMS_GO(0, 1);
     else if (out == 0) RMS_GO(1, 0);
@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(128) fp32_sincos_kernel(
             long long p = p0 + j;
             int ch = c0 + c;
             float q = 0.f, u = 0.f;
-            if (p < n_pix && ch < n_chan) {
+            if (p < n_pix && ch < n_chan && kwf[ch] != 0.f) {   // reading A13: zero-weight channels are never read
                 size_t off = IN == 0 ? (size_t)p * n_chan + ch : (size_t)ch * n_pix + p;
                 q = Q[off];
                 u = U[off];

@@ -192,6 +192,7 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
         return fail(RMSYNTH_EINVAL, "unknown scheme");
     if (o.lambda0_mode < 0 || o.lambda0_mode > 2) return fail(RMSYNTH_EINVAL, "unknown lambda0_mode");
     if (o.lambda0_mode == 2 && !std::isfinite(o.lambda0_sq)) return fail(RMSYNTH_EINVAL, "lambda0_sq not finite");
+    if (o.host_chunk_pixels < 0) return fail(RMSYNTH_EINVAL, "host_chunk_pixels < 0");
 
     rmsynth_plan* p = new (std::nothrow) rmsynth_plan;
     if (!p) return fail(RMSYNTH_ENOMEM, "plan");
@@ -199,6 +200,7 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
     p->n_phi = n_phi;
     p->scheme = scheme;
     p->lambda0_mode = o.lambda0_mode;
+    p->host_chunk_pixels = o.host_chunk_pixels;
     const double c = 299792458.0;
     double W = 0.0, S = 0.0, M = 0.0;
     p->lam2.resize(n_chan);
@@ -229,8 +231,10 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
     p->K = 1.0 / W;
     p->lambda0_sq = o.lambda0_mode == 0 ? S / W : (o.lambda0_mode == 1 ? M / n_chan : o.lambda0_sq);
 
+    DeviceGuard guard(o.device);                       // the plan's device for the rest of this call, the caller's afterwards
     int dev = o.device;
-    cudaError_t e = dev < 0 ? cudaGetDevice(&dev) : cudaSetDevice(dev);
+    cudaError_t e = guard.err;
+    if (e == cudaSuccess && dev < 0) e = cudaGetDevice(&dev);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
     if (e != cudaSuccess) {
@@ -256,6 +260,7 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
 
 rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
     if (!p) return RMSYNTH_OK;
+    DeviceGuard guard(p->device);
     tc_plan_free(p);
     void* ptrs[] = {p->d_delta, p->d_kw, p->d_phi, p->d_cos, p->d_sin, p->d_phif, p->d_kwf, p->d_dpi, p->d_phi2};
     for (void* q : ptrs)
@@ -264,8 +269,7 @@ rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
         if (p->scratch[i]) cudaFree(p->scratch[i]);
     for (auto& x : p->pool)
         if (x.ptr) cudaFree(x.ptr);
-    for (int i = 0; i < 2; ++i)
-        if (p->hs[i]) cudaStreamDestroy(p->hs[i]);
+    host_pipe_free(p);
     delete p;
     return RMSYNTH_OK;
 }
@@ -283,6 +287,8 @@ rmsynth_status rmsynth_plan_info(const rmsynth_plan* p, double* lambda0_sq, doub
 
 rmsynth_status rmsynth_plan_phase_matrix(const rmsynth_plan* p, float* cos_kw, float* sin_kw) {
     if (!p) return fail(RMSYNTH_EINVAL, "plan is NULL");
+    DeviceGuard guard(p->device);
+    RMS_CUDA(guard.err);
     size_t row = sizeof(float) * p->n_phi;
     if (cos_kw)
         RMS_CUDA(cudaMemcpy2D(cos_kw, row, p->d_cos, sizeof(float) * p->ldb, row, p->n_chan, cudaMemcpyDeviceToHost));
@@ -303,7 +309,8 @@ rmsynth_status rmsynth_rmsf(const rmsynth_plan* p, const double* phi_eval, int n
     if (n == 0) return RMSYNTH_OK;
     for (int k = 0; k < n; ++k)
         if (!std::isfinite(phi_eval[k])) return fail(RMSYNTH_EINVAL, "phi_eval must be finite");
-    RMS_CUDA(cudaSetDevice(p->device));
+    DeviceGuard guard(p->device);
+    RMS_CUDA(guard.err);
     double* d_phi = nullptr;
     RMS_CUDA(cudaMalloc(&d_phi, sizeof(double) * n));
     cudaError_t e = cudaMemcpy(d_phi, phi_eval, sizeof(double) * n, cudaMemcpyHostToDevice);

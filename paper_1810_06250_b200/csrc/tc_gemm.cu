@@ -44,16 +44,23 @@ rmsynth_status tc_plan_init(rmsynth_plan* p) {
     g.k_pad = n_stages * TC_KS;
     g.ctas = 2;
     if (!get_encode_fn()) return fail(RMSYNTH_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+    // reading A13: channels with w = 0 are removed -- both tensor kernels zero their samples on the way in
+    const int n_words = (p->n_chan + 31) / 32;
+    std::vector<uint32_t> mask(n_words, 0u);
+    for (int i = 0; i < p->n_chan; ++i)
+        if (p->w[i] > 0.0) mask[i / 32] |= 1u << (i % 32);
+    RMS_CUDA(cudaMalloc(&p->d_chanmask, sizeof(uint32_t) * n_words));
+    RMS_CUDA(cudaMemcpy(p->d_chanmask, mask.data(), sizeof(uint32_t) * n_words, cudaMemcpyHostToDevice));
     return p->scheme == RMSYNTH_SCHEME_F16X3 ? tc3_plan_init(p) : tc2_plan_init(p);
 }
 
 void tc_plan_free(rmsynth_plan* p) {
     if (p->d_tcB2) cudaFree(p->d_tcB2);
     if (p->d_tcB3) cudaFree(p->d_tcB3);
-    if (p->d_tc3mask) cudaFree(p->d_tc3mask);
+    if (p->d_chanmask) cudaFree(p->d_chanmask);
     p->d_tcB2 = nullptr;
     p->d_tcB3 = nullptr;
-    p->d_tc3mask = nullptr;
+    p->d_chanmask = nullptr;
 }
 
 // Copy a cube into a buffer whose row pitch is a multiple of 4 floats (TMA needs 16-byte strides).

@@ -85,6 +85,7 @@ struct Tc2Params {
     int* tile_sync;      // [pixel-tile pairs] check-in counters (gang_checkin), NULL = off
     int gang;                     // gang size G of the work schedule (tc_common.cuh: WorkIter)
     int sync_lag;        // gang members may drift this many work items apart
+    const uint32_t* chan_mask;   // per 32 channels: bit i set = channel exists and has w > 0
 };
 
 template <int IN_MN, int OUT_LOS>
@@ -227,13 +228,31 @@ tc2_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             int tp, j;
             while (wi.next(tp, j)) total += prm.n_stages;
         }
+        int stage = 0;                                       // 8-channel stage within the work item
         for (long long it = 0; it < total; ++it) {
             mbar_wait(&full[st], ph);
             uint8_t* sg = smem_gen + (size_t)st * T2_STAGE;
+            // reading A13: zero-weight channels are removed -- their samples (NaN-blanked planes included) become zeros
+            // in the raw tile (= A_hi) and in A_lo.  Warp-uniform: stages without a flagged channel skip all of it.
+            const uint32_t m8 = (__ldg(prm.chan_mask + (stage >> 2)) >> ((stage & 3) * 8)) & 0xFFu;
+            if (++stage == prm.n_stages) stage = 0;
 #pragma unroll
             for (int v = 0; v < 2 * T2_APART / 16 / 128; ++v) {
                 const int o = (v * 128 + tt) * 16;
                 float4 a = *reinterpret_cast<const float4*>(sg + o);
+                if (m8 != 0xFFu) {
+                    const int oo = o & (T2_APART - 1);           // offset inside the Q or the U part
+                    if (IN_MN) {                                 // [pixel group][channel][32 pixels]: a unit belongs to one channel
+                        if (!((m8 >> ((oo >> 7) & 7)) & 1u)) a = make_float4(0.f, 0.f, 0.f, 0.f);
+                    } else {                                     // [pixel][8 channels], SWIZZLE_32B: unit j' holds channels 4 (j' ^ bit 2 of the row) ..
+                        const int c0 = ((((oo >> 4) & 1) ^ ((oo >> 7) & 1)) << 2);
+                        if (!((m8 >> c0) & 1u)) a.x = 0.f;
+                        if (!((m8 >> (c0 + 1)) & 1u)) a.y = 0.f;
+                        if (!((m8 >> (c0 + 2)) & 1u)) a.z = 0.f;
+                        if (!((m8 >> (c0 + 3)) & 1u)) a.w = 0.f;
+                    }
+                    *reinterpret_cast<float4*>(sg + o) = a;
+                }
                 float4 l;
                 auto lo = [](float x) {
                     float h = __uint_as_float(__float_as_uint(x) & 0xFFFFE000u);
@@ -343,6 +362,7 @@ rmsynth_status tc2_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.tile_sync = tile_sync;
     prm.gang = gang;
     prm.sync_lag = sync_lag;
+    prm.chan_mask = p->d_chanmask;
     const int max_clusters = p->sm_count / 2;
     const int clusters = prm.n_items < max_clusters ? prm.n_items : max_clusters;
     const int grid = 2 * clusters;

@@ -596,11 +596,6 @@ rmsynth_status tc3_plan_init(rmsynth_plan* p) {
     int eb;
     std::frexp(bmax, &eb);                       // bmax = f 2^eb, f in [0.5, 1)
     p->tc3_eb = 15 - eb;                         // bmax 2^(15 - eb) in [2^14, 2^15)
-    std::vector<uint32_t> mask(n_chunks, 0u);
-    for (int i = 0; i < p->n_chan; ++i)
-        if (p->w[i] > 0.0) mask[i / T3_KC] |= 1u << (i % T3_KC);
-    RMS_CUDA(cudaMalloc(&p->d_tc3mask, sizeof(uint32_t) * n_chunks));
-    RMS_CUDA(cudaMemcpy(p->d_tc3mask, mask.data(), sizeof(uint32_t) * n_chunks, cudaMemcpyHostToDevice));
     const size_t halves = (size_t)g.n_phi_tiles * n_chunks * 2 * 128 * g.n_tile;
     RMS_CUDA(cudaMalloc(&p->d_tcB3, halves * sizeof(__half)));
     dim3 grid((g.n_tile + 63) / 64, n_chunks, g.n_phi_tiles);
@@ -630,7 +625,7 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.a3d = a3d ? 1 : 0;
     prm.inv_scale_b = (float)std::ldexp(1.0, -p->tc3_eb);
     prm.blob = reinterpret_cast<const __half*>(p->d_tcB3);
-    prm.chan_mask = p->d_tc3mask;
+    prm.chan_mask = p->d_chanmask;
     prm.FQ = FQ;
     prm.FU = FU;
     prm.FA = FA;

@@ -175,10 +175,15 @@ def test_concurrent_streams_share_a_plan(b, oracle_mod):
                 plan.execute_peaks(dq, du, 3000, 0, fq, fu, peak_index=idx, stream=s.cuda_stream)
             outs.append((fq, fu, idx))
     torch.cuda.synchronize()
-    ref = oracle_mod.peaks(op, FQ, FU)["kstar"]
+    y = np.sqrt(FQ ** 2 + FU ** 2)
+    ko = oracle_mod.peaks(op, FQ, FU)["kstar"].astype(np.int64)
+    rows = np.arange(3000)
     for fq, fu, idx in outs:
         check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, "concurrent streams")
-        assert (idx.cpu().numpy() == ref).mean() > 0.99
+        kg = idx.cpu().numpy().astype(np.int64)
+        assert kg.min() >= 0 and kg.max() < plan.n_phi
+        # the index rule of check_peaks: equal, unless the oracle's |F| at the two depths differ by <= 2e-5 T_p
+        assert not ((kg != ko) & (y[rows, ko] - y[rows, kg] > 2 * TOL * T)).any()
     plan.destroy()
 
 
@@ -217,13 +222,19 @@ def test_flagged_channels_full_of_interference(b, oracle_mod, scheme):
     q, u = q.copy(), u.copy()
     q[::3, flagged[::2]] = 1e30
     u[1::3, flagged[1::2]] = -3e28
+    # reading A13: a flagged channel is REMOVED, so NaN-blanked / overflowed planes are as harmless as finite garbage
+    q[5::7, flagged[3]] = np.nan
+    u[2::5, flagged[10]] = np.inf
+    q[:, flagged[20]] = -np.inf
+    u[:, flagged[21]] = np.nan
     _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
     assert np.all(np.isfinite(FQ)) and np.all(T < 10)
     plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
     out = run_gpu(b, plan, q, u, "freq", "phi")
     check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} flagged garbage")
-    out = run_gpu(b, plan, q, u, "los", "los")
+    out = run_gpu(b, plan, q, u, "los", "los", peaks=True)
     check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"{scheme} flagged garbage los")
+    assert out["maps"]["kstar"].min() >= 0 and np.all(np.isfinite(out["maps"]["peak_amp"]))
     plan.destroy()
 
 
@@ -336,6 +347,103 @@ def test_execute_host_matches_oracle(b, oracle_mod, scheme, lin, lout):
     plan.destroy()
 
 
+@pytest.mark.parametrize("scheme", ["f16x3", "tf32x3", "fp32_table"])
+@pytest.mark.parametrize("lin,lout", LAYOUTS)
+def test_execute_host_multi_chunk(b, oracle_mod, scheme, lin, lout):
+    """The three-slot pipeline proper: 7 chunks of 148 lines of sight with a ragged last one (997 = 6 x 148 + 109;
+    109 % 4 != 0 -> the repack path), slot re-use after three chunks, column-sliced 2-D copies for the FITS-order and
+    phi-major layouts, map offsets -- cubes + maps, then maps only (no cube crosses the bus)."""
+    cfg, nu, w, phi, q, u = inputs(4, 997, start=5)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme], host_chunk_pixels=148)
+    out = run_gpu(b, plan, q, u, lin, lout, peaks=True, host=True)
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, f"execute_host 7 chunks {scheme} {lin}->{lout}")
+    check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], cfg.dphi, "execute_host 7 chunks")
+    out2 = run_gpu(b, plan, q, u, lin, lout, peaks=True, cubes=False, host=True)
+    check_peaks(oracle_mod, op, FQ, FU, T, out2["maps"], cfg.dphi, "execute_host 7 chunks, maps only")
+    plan.destroy()
+
+
+def test_execute_host_on_a_7000_depth_grid(b, oracle_mod):
+    """The paper's LOFAR shape of the depth axis (856 channels -> 7000 depths): 68 depth tiles per pixel tile,
+    streamed in 5 chunks through the host path."""
+    cfg = ri.CONFIGS[7]
+    nu, w, phi = ri.grids(cfg)
+    assert phi.size == 7000 and nu.size == 856
+    q, u = ri.generate_pixels(cfg, torch.arange(11, 11 + 600))
+    q, u = q.numpy(), u.numpy()
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    plan = b.Plan(nu, w, phi, host_chunk_pixels=128)
+    out = run_gpu(b, plan, q, u, "freq", "phi", peaks=True, host=True)
+    check_cubes(out["FQ"], out["FU"], FQ, FU, T, "execute_host 7000 depths")
+    check_peaks(oracle_mod, op, FQ, FU, T, out["maps"], cfg.dphi, "execute_host 7000 depths")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("lin,lout", [("freq", "phi"), ("los", "los")])
+@pytest.mark.parametrize("want", ["cubes+maps", "maps"])
+def test_execute_stream_callbacks(b, oracle_mod, lin, lout, want):
+    """rmsynth_execute_stream: the caller refills pinned staging chunk by chunk (the out-of-core form for cubes that
+    do not fit in host memory): 6 chunks of 200 with a ragged last one, every chunk handed back exactly once
+    and in order, results equal to the oracle's."""
+    cfg, nu, w, phi, q, u = inputs(2, 1090, start=3)
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    n_pix, n_chan, n_phi = q.shape[0], q.shape[1], phi.size
+    plan = b.Plan(nu, w, phi, host_chunk_pixels=200)
+    layout = (b.IN_FREQ_MAJOR if lin == "freq" else 0) | (b.OUT_PHI_MAJOR if lout == "phi" else 0)
+    got_q = np.full((n_pix, n_phi), np.nan, np.float32)
+    got_u = np.full_like(got_q, np.nan)
+    maps = {k: np.full(n_pix, np.nan, np.float32) for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero")}
+    maps["kstar"] = np.full(n_pix, -7, np.int32)
+    order, starts = [], {}
+
+    def fill(i, Q, U, max_pix):
+        assert max_pix == 200
+        p0 = i * 200
+        n = max(0, min(200, n_pix - p0))
+        if n:
+            starts[i] = p0
+            blk_q, blk_u = q[p0:p0 + n], u[p0:p0 + n]
+            Q[:n * n_chan] = (blk_q.T if lin == "freq" else blk_q).ravel()
+            U[:n * n_chan] = (blk_u.T if lin == "freq" else blk_u).ravel()
+        return n
+
+    def drain(i, n, out):
+        order.append(i)
+        p0 = starts[i]
+        if want == "cubes+maps":
+            shape = (n_phi, n) if lout == "phi" else (n, n_phi)
+            fq, fu = out["FQ"].reshape(shape), out["FU"].reshape(shape)
+            got_q[p0:p0 + n] = fq.T if lout == "phi" else fq
+            got_u[p0:p0 + n] = fu.T if lout == "phi" else fu
+        else:
+            assert "FQ" not in out
+        for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+            maps[k][p0:p0 + n] = out[k]
+        maps["kstar"][p0:p0 + n] = out["peak_index"]
+
+    done = plan.execute_stream(layout, (b.WANT_CUBES if want == "cubes+maps" else 0) | b.WANT_MAPS, fill, drain)
+    assert done == n_pix and order == list(range(6))
+    if want == "cubes+maps":
+        check_cubes(got_q, got_u, FQ, FU, T, f"execute_stream {lin}->{lout}")
+    check_peaks(oracle_mod, op, FQ, FU, T, maps, cfg.dphi, f"execute_stream {want}")
+    plan.destroy()
+
+
+def test_plan_device_is_honoured_and_current_device_left_alone(b):
+    """A plan runs on the device it was created for and the calls leave the caller's current device as they found it."""
+    nu, phi = np.linspace(1e9, 2e9, 16), np.linspace(-10, 10, 5)
+    before = torch.cuda.current_device()
+    plan = b.Plan(nu, None, phi, device=0)
+    q = torch.randn(8, 16, device="cuda:0")
+    f = torch.zeros(8, 5, device="cuda:0")
+    plan.execute(q, q, 8, 0, f, f)
+    plan.rmsf(np.array([0.5]))
+    torch.cuda.synchronize()
+    assert torch.cuda.current_device() == before and torch.isfinite(f).all()
+    plan.destroy()
+
+
 def test_api_edges(b):
     nu, phi = np.linspace(1e9, 2e9, 16), np.linspace(-10, 10, 5)
     for scheme in SCHEMES:
@@ -411,9 +519,38 @@ def test_nonfinite_samples_stay_in_their_pixel(b):
         plan.destroy()
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("lin,lout,n_pix", [("freq", "phi", 520), ("los", "los", 300), ("freq", "phi", 389)])
+def test_nonfinite_lines_of_sight_in_the_peak_maps(b, oracle_mod, scheme, lin, lout, n_pix):
+    """Reading A17: a line of sight with a non-finite |F| has no peak -- index -1 and NaN in every map, with the cubes
+    written and in a maps-only call alike; its neighbours are untouched (520 and 300 pixels take the FP16 kernel's
+    fast tile ends, 389 the scalar one)."""
+    cfg, nu, w, phi, q, u = inputs(5, n_pix, start=1)
+    q, u = q.copy(), u.copy()
+    bad = [0, 31, 32, 127, 128, n_pix - 1, n_pix // 2]
+    for j, pix in enumerate(bad):
+        (q if j % 2 else u)[pix, (37 * j) % cfg.n_chan] = [np.nan, np.inf, -np.inf][j % 3]
+    op, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    ref = oracle_mod.peaks(op, FQ, FU)
+    assert sorted(np.flatnonzero(ref["kstar"] < 0).tolist()) == sorted(bad)
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    good = np.setdiff1d(np.arange(n_pix), bad)
+    for cubes in (True, False):
+        out = run_gpu(b, plan, q, u, lin, lout, peaks=True, cubes=cubes)
+        m = out["maps"]
+        assert np.all(m["kstar"][bad] == -1) and np.all(m["kstar"][good] >= 0), f"{scheme} cubes={cubes}"
+        for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero"):
+            assert np.all(np.isnan(m[k][bad])) and np.all(np.isfinite(m[k][good])), (scheme, cubes, k)
+        check_peaks(oracle_mod, op, FQ, FU, T, m, cfg.dphi, f"{scheme} non-finite maps cubes={cubes}")
+        if cubes:
+            check_cubes(out["FQ"][good], out["FU"][good], FQ[good], FU[good], T[good], f"{scheme} finite neighbours")
+            assert np.all(np.isnan(out["FQ"][bad]) | np.isinf(out["FQ"][bad]))
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ full BASELINE sizes, bench launch configuration
-@pytest.mark.parametrize("cfg_id", [2, 4, 3, 5])
-def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id):
+@pytest.mark.parametrize("cfg_id,scheme", [(2, "auto"), (4, "auto"), (3, "auto"), (5, "auto"), (2, "tf32x3"), (5, "tf32x3")])
+def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id, scheme):
     """The cube bench.py times (same layouts, same scheme, one rmsynth_execute_peaks call over the whole
     cube), checked on lines of sight the oracle can compute one by one: every pixel of the first and last
     tile, tile-boundary neighbours and a random sample; plus properties that hold at any size."""
@@ -426,7 +563,8 @@ def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id):
     FU = torch.full(shape, float("nan"), device="cuda")
     maps = {k: torch.full((cfg.n_pix,), float("nan"), device="cuda") for k in ("peak_amp", "peak_phi", "pa_lambda0", "pa_zero")}
     maps["peak_index"] = torch.full((cfg.n_pix,), -1, dtype=torch.int32, device="cuda")
-    plan = b.Plan(nu, w, phi)                                   # default scheme = the product path
+    # default scheme = the product path; 3xTF32 = what AUTO falls back to (few channels, wide weight spans)
+    plan = b.Plan(nu, w, phi, scheme=b.SCHEME_AUTO if scheme == "auto" else b.SCHEME_TF32X3)
     plan.execute_peaks(Q, U, cfg.n_pix, layout, FQ, FU, **maps)
     torch.cuda.synchronize()
     # properties at full size: every output written and finite, |F| <= T_p (triangle inequality), index in range
