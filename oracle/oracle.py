@@ -48,6 +48,9 @@ def _load():
         lib.oracle_tolerance_scale.restype = None
         lib.oracle_peaks.argtypes = [dp, dp, C.c_longlong, dp, C.c_int, C.c_double, ip, dp, dp, dp, dp]
         lib.oracle_peaks.restype = None
+        lib.oracle_rmclean.argtypes = [dp, dp, C.c_longlong, C.c_int, dp, dp, C.c_double, C.c_double, C.c_int,
+                                       C.c_double, C.c_double, dp, dp, dp, dp, dp, dp, ip, dp]
+        lib.oracle_rmclean.restype = None
         _lib = lib
     return _lib
 
@@ -152,3 +155,33 @@ def peaks(plan: Plan, FQ, FU):
     _load().oracle_peaks(_d(FQ), _d(FU), n, _d(plan.phi), plan.phi.size, plan.lambda0_sq,
                          k.ctypes.data_as(C.POINTER(C.c_int)), _d(amp), _d(ph), _d(pa0), _d(paz))
     return dict(kstar=k, peak_amp=amp, peak_phi=ph, pa_lambda0=pa0, pa_zero=paz)
+
+
+def rmsf_double_width(plan: Plan):
+    """R on the double-width grid of reading C1: R(m dphi), m = -(n_phi-1) .. n_phi-1 (uniform plan grid required)."""
+    n = plan.phi.size
+    dphi = (plan.phi[-1] - plan.phi[0]) / (n - 1) if n > 1 else 1.0
+    if n > 2 and np.max(np.abs(np.diff(plan.phi) - dphi)) > 1e-9 * abs(dphi):
+        raise ValueError("RM-CLEAN needs a uniform depth grid (reading C1)")
+    return rmsf(plan, np.arange(-(n - 1), n) * dphi), dphi
+
+
+def rmclean(plan: Plan, FQ, FU, gain=0.1, cutoff=0.0, max_iter=100, fwhm=None, restore=True):
+    """Hogbom RM-CLEAN per line of sight (readings C1-C8).  FQ, FU: dirty cubes [n_pix, n_phi] (any float type, promoted
+    to FP64).  Returns dict(model, residual, restored (or None), n_iter, min_margin); cubes complex128 [n_pix, n_phi]."""
+    FQ, FU = _f64(FQ), _f64(FU)
+    n_pix, n_phi = FQ.shape
+    assert n_phi == plan.phi.size
+    R, dphi = rmsf_double_width(plan)
+    Rre, Rim = _f64(R.real), _f64(R.imag)
+    mq, mu, rq, ru = (np.empty((n_pix, n_phi)) for _ in range(4))
+    sq, su = (np.empty((n_pix, n_phi)), np.empty((n_pix, n_phi))) if restore else (None, None)
+    it = np.empty(n_pix, dtype=np.int32)
+    margin = np.empty(n_pix)
+    null = C.POINTER(C.c_double)()
+    _load().oracle_rmclean(_d(FQ), _d(FU), n_pix, n_phi, _d(Rre), _d(Rim), float(gain), float(cutoff), int(max_iter),
+                           float(dphi), float(fwhm if fwhm is not None else 1.0),
+                           _d(mq), _d(mu), _d(rq), _d(ru), _d(sq) if restore else null, _d(su) if restore else null,
+                           it.ctypes.data_as(C.POINTER(C.c_int)), _d(margin))
+    return dict(model=mq + 1j * mu, residual=rq + 1j * ru, restored=(sq + 1j * su) if restore else None,
+                n_iter=it, min_margin=margin)

@@ -13,6 +13,9 @@
  *
  * Pin status (tests/test_oracle_pins.py):
  *   lambda^2, K, lambda0^2, F (naive + table), R, T_p, k*  : pinned (P1-P11, P13)
+ *   RM-CLEAN loop (oracle_rmclean, readings C1-C8)         : pinned (C-pins: exact
+ *     decomposition identity, geometric series of an on-grid point source, two
+ *     separated sources, zero iterations, threshold stop)
  *   parabolic refinement, PA maps (A8-A10)                 : pinned by P12 only
  *     (exact parabola, on-grid point source); the paper prints no worked
  *     example for them -> "parity unpinned" beyond P12.
@@ -244,5 +247,96 @@ void oracle_peaks(const double *FQ, const double *FU, long long n_pix,
         double pa = 0.5 * atan2(fu[kb], fq[kb]);
         pa_lambda0[p] = pa;
         pa_zero[p] = wrap_half_pi(pa - ph * lambda0_sq);
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * RM-CLEAN per line of sight (scope row NEXT-3).  The paper only NAMES the
+ * procedure: "Equation 12 is needed only if one wishes to deconvolve R(phi)
+ * from the reconstructed Faraday dispersion function using a procedure called
+ * RM-CLEAN (Heald 2009)" (footnote 6).  Every step
+ * below is therefore a READING, listed as C1-C8 in DESIGN.md section 2b: a
+ * Hogbom CLEAN of the complex dirty spectrum F~(phi_k) with the complex RMSF
+ * as the beam ("F~ is equivalent to the dirty image and R to the dirty
+ * beam").
+ *
+ *   C1  the depth grid is uniform, phi_k = phi_0 + k dphi, so the beam centred
+ *       on sample j is R((k - j) dphi): R is given on the DOUBLE-WIDTH grid
+ *       Rdw[m], m = -(n_phi-1) .. n_phi-1, stored at index m + n_phi - 1
+ *       (2 n_phi - 1 complex samples; R(0) = 1 by Eq. 12-13).
+ *   C2  residual r <- F~ (complex), model m <- 0 (complex, on the same grid).
+ *   C3  each iteration: k* = lowest index of the maximum of |r_k|; stop BEFORE
+ *       subtracting if |r_k*| < cutoff (absolute, in the units of F) or if
+ *       max_iter iterations have been done.
+ *   C4  component c = gain * r_k* (complex); m_k* += c;
+ *       r_k -= c * Rdw[k - k*]  for every k (complex multiply).
+ *   C5  restored spectrum = sum_j m_j G((k - j) dphi) + r_k with the REAL
+ *       Gaussian G(x) = exp(-x^2 / (2 sigma^2)), sigma = fwhm / (2 sqrt(2 ln 2)),
+ *       fwhm = the caller's value (the FWHM of |R|).
+ *   C6  outputs: model (complex), residual (complex), restored (complex, may be
+ *       NULL), number of iterations done, and min_margin = the smallest value,
+ *       over the iterations, of |r_k*| - (second largest |r_k|): how close the
+ *       arg-max decision ever came to a tie (for parity rules, not part of the
+ *       algorithm).
+ *   C7  a line of sight with a non-finite sample is left alone: model 0,
+ *       residual = input, restored = input, iterations 0 (reading A17).
+ *   C8  FP64 throughout; FQ, FU are the FP64 dirty cubes, LOS-major.
+ */
+void oracle_rmclean(const double *FQ, const double *FU, long long n_pix, int n_phi,
+                    const double *Rdw_re, const double *Rdw_im,
+                    double gain, double cutoff, int max_iter,
+                    double dphi, double fwhm,
+                    double *model_q, double *model_u,
+                    double *resid_q, double *resid_u,
+                    double *rest_q, double *rest_u,
+                    int *n_iter, double *min_margin)
+{
+    const int c0 = n_phi - 1; /* index of R(0) in the double-width array */
+    for (long long p = 0; p < n_pix; ++p) {
+        const double *fq = FQ + p * n_phi, *fu = FU + p * n_phi;
+        double *mq = model_q + p * n_phi, *mu = model_u + p * n_phi;
+        double *rq = resid_q + p * n_phi, *ru = resid_u + p * n_phi;
+        int finite = 1;
+        for (int k = 0; k < n_phi; ++k) {
+            mq[k] = 0.0; mu[k] = 0.0;
+            rq[k] = fq[k]; ru[k] = fu[k];
+            if (!isfinite(fq[k]) || !isfinite(fu[k])) finite = 0;
+        }
+        int it = 0;
+        double margin = INFINITY;
+        while (finite && it < max_iter) {
+            int kb = 0;
+            double yb = -1.0, y2nd = -1.0;
+            for (int k = 0; k < n_phi; ++k) {
+                double y = sqrt(rq[k] * rq[k] + ru[k] * ru[k]);
+                if (y > yb) { y2nd = yb; yb = y; kb = k; }
+                else if (y > y2nd) y2nd = y;
+            }
+            if (yb < cutoff) break;                              /* C3 */
+            if (n_phi > 1 && yb - y2nd < margin) margin = yb - y2nd;
+            double cq = gain * rq[kb], cu = gain * ru[kb];       /* C4 */
+            mq[kb] += cq; mu[kb] += cu;
+            for (int k = 0; k < n_phi; ++k) {
+                double br = Rdw_re[c0 + k - kb], bi = Rdw_im[c0 + k - kb];
+                rq[k] -= cq * br - cu * bi;
+                ru[k] -= cq * bi + cu * br;
+            }
+            ++it;
+        }
+        n_iter[p] = it;
+        if (min_margin) min_margin[p] = margin;
+        if (rest_q && rest_u) {                                  /* C5 */
+            const double sigma = fwhm / (2.0 * sqrt(2.0 * log(2.0)));
+            for (int k = 0; k < n_phi; ++k) {
+                double sq = rq[k], su = ru[k];
+                for (int j = 0; j < n_phi; ++j) {
+                    if (mq[j] == 0.0 && mu[j] == 0.0) continue;
+                    double x = (double)(k - j) * dphi;
+                    double g = exp(-x * x / (2.0 * sigma * sigma));
+                    sq += mq[j] * g; su += mu[j] * g;
+                }
+                rest_q[p * n_phi + k] = sq; rest_u[p * n_phi + k] = su;
+            }
+        }
     }
 }
