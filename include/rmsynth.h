@@ -170,6 +170,32 @@ rmsynth_status rmsynth_execute_stream(const rmsynth_plan *plan, int layout, int 
                                       rmsynth_fill_fn fill, rmsynth_drain_fn drain, void *user,
                                       long long *n_pix_done);
 
+/* RM-CLEAN per line of sight (the deconvolution the paper names as the use of Eq. 12, footnote 6
+ * the paper defines no step of it; the loop is reading C1-C8 of DESIGN.md): Hogbom CLEAN
+ * of the complex dirty spectrum F~ = FQ + i FU with the complex RMSF as the beam.
+ *   r <- F~, m <- 0; repeat up to max_iter times: k* = lowest index of max |r_k|; stop if |r_k*| < cutoff;
+ *   c = gain r_k*; m_k* += c; r_k -= c R(phi_k - phi_k*) for all k.
+ *   restored_k = sum_j m_j G(phi_k - phi_j) + r_k, G a real Gaussian of FWHM `fwhm` (<= 0: the FWHM of |R|).
+ *   FQ, FU            DEVICE dirty cubes, n_pix*n_phi floats each, laid out per the RMSYNTH_OUT_* bit of `layout`
+ *                     (what rmsynth_execute wrote); the RMSYNTH_IN_* bit is ignored
+ *   model_*, resid_*  DEVICE output cubes, same layout; rest_* likewise or both NULL
+ *   n_iter            DEVICE [n_pix] iterations done per line of sight, or NULL
+ * A line of sight holding a non-finite sample is passed through (model 0, residual = restored = input, 0
+ * iterations).  Needs a uniform depth grid (else EUNSUPPORTED) of at most 14080 depths.  Only enqueues on
+ * `stream`, except the first call of a plan (and a change of fwhm), which builds the beam synchronously.
+ * EINVAL: gain outside (0, 1], cutoff < 0, max_iter < 0, NULL cubes. */
+typedef struct {
+    int struct_size;   /* sizeof(rmsynth_clean_params) */
+    float gain;
+    float cutoff;      /* absolute, in the units of F */
+    int max_iter;
+    float fwhm;        /* rad m^-2; <= 0 = FWHM of |R| measured on the plan's grid */
+} rmsynth_clean_params;
+rmsynth_status rmsynth_rmclean(const rmsynth_plan *plan, const float *FQ, const float *FU, long long n_pix,
+                               int layout, const rmsynth_clean_params *params, float *model_q,
+                               float *model_u, float *resid_q, float *resid_u, float *rest_q,
+                               float *rest_u, int *n_iter, void *stream);
+
 /* R(phi) of Eq. 12 in FP64.  phi_eval HOST [n] or NULL for the plan grid (then n must be
  * n_phi); R_re, R_im HOST [n].  Synchronous. */
 rmsynth_status rmsynth_rmsf(const rmsynth_plan *plan, const double *phi_eval, int n,

@@ -27,7 +27,7 @@ SCHEME_AUTO, SCHEME_TF32X3, SCHEME_F16X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS 
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
            "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_execute_stream",
-           "rmsynth_rmsf",
+           "rmsynth_rmsf", "rmsynth_rmclean",
            "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
 
 
@@ -55,6 +55,13 @@ FILL_FN = C.CFUNCTYPE(C.c_longlong, C.c_void_p, C.c_longlong, C.c_void_p, C.c_vo
 DRAIN_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_longlong, C.c_longlong, C.POINTER(Outputs))
 WANT_CUBES, WANT_MAPS = 1, 2
 _lib.rmsynth_execute_stream.argtypes = [_vp, C.c_int, C.c_int, FILL_FN, DRAIN_FN, C.c_void_p, C.POINTER(C.c_longlong)]
+
+
+class CleanParams(C.Structure):
+    _fields_ = [("struct_size", C.c_int), ("gain", C.c_float), ("cutoff", C.c_float), ("max_iter", C.c_int), ("fwhm", C.c_float)]
+
+
+_lib.rmsynth_rmclean.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, C.POINTER(CleanParams), _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
 _lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
 _lib.rmsynth_launch_count.argtypes = [C.c_int]
 _lib.rmsynth_launch_count.restype = C.c_longlong
@@ -162,6 +169,13 @@ class Plan:
         _check(_lib.rmsynth_execute_host(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
                                          _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
                                          _ptr(peak_index)))
+
+    def rmclean(self, FQ, FU, n_pix, layout, gain, cutoff, max_iter, model_q, model_u, resid_q, resid_u,
+                rest_q=None, rest_u=None, n_iter=None, fwhm=0.0, stream=None):
+        """RM-CLEAN of device-resident dirty cubes (all DEVICE tensors, laid out per the OUT_* bit of `layout`)."""
+        prm = CleanParams(C.sizeof(CleanParams), gain, cutoff, max_iter, fwhm)
+        _check(_lib.rmsynth_rmclean(self._h, _ptr(FQ), _ptr(FU), n_pix, layout, C.byref(prm), _ptr(model_q), _ptr(model_u),
+                                    _ptr(resid_q), _ptr(resid_u), _ptr(rest_q), _ptr(rest_u), _ptr(n_iter), stream))
 
     def execute_stream(self, layout, outputs, fill, drain):
         """fill(i, Q, U, max_pix) -> n and drain(i, n, out) are Python callables; Q, U are numpy views of the

@@ -98,6 +98,14 @@ struct rmsynth_plan {
     mutable std::vector<StreamScratch> pool;
     mutable void* host_pipe = nullptr;    // streams, events and staging of the host-streaming engine (execute.cu)
     long long host_chunk_pixels = 0;      // rmsynth_options.host_chunk_pixels (0 = automatic)
+    // RM-CLEAN (rmclean.cu): needs a uniform depth grid; beam and restoring Gaussian are built on first use
+    bool uniform_phi = false;
+    double dphi = 0.0;
+    mutable float2* d_Rdw = nullptr;      // R((k - j) dphi), 2 n_phi - 1 samples, R(0) at n_phi - 1
+    mutable float* d_gauss = nullptr;     // restoring Gaussian at m dphi, m = 0 .. n_phi - 1
+    mutable float gauss_fwhm = 0.f;
+    mutable int gauss_reach = 0;
+    mutable double rmsf_fwhm = 0.0;       // FWHM of |R| (used when the caller passes fwhm <= 0)
 };
 
 namespace rms {

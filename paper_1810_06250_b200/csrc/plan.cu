@@ -94,6 +94,13 @@ __global__ void rmsf_kernel(const double* __restrict__ delta, const double* __re
     if (lane == 0) { re[k] = sr; im[k] = si; }
 }
 
+// R(phi) for n device-resident depths into device arrays (used by rmclean.cu for the double-width beam)
+rmsynth_status device_rmsf_to(const rmsynth_plan* p, const double* d_phi, int n, double* d_re, double* d_im) {
+    rmsf_kernel<<<(n + 3) / 4, 128>>>(p->d_delta, p->d_kw, d_phi, p->n_chan, n, d_re, d_im);
+    RMS_LAUNCH_CHECK("rmsf_kernel");
+    return RMSYNTH_OK;
+}
+
 static rmsynth_status device_rmsf(const rmsynth_plan* p, const double* d_phi, int n, double* re, double* im) {
     double* d_out = nullptr;
     RMS_CUDA(cudaMalloc(&d_out, sizeof(double) * 2 * (size_t)n));
@@ -228,6 +235,11 @@ rmsynth_status rmsynth_plan_create(rmsynth_plan** plan, const double* nu_hz, con
             delete p;
             return fail(RMSYNTH_EINVAL, "phi must be finite");
         }
+    // uniform grid? (RM-CLEAN shifts one beam along the grid, reading C1)
+    p->dphi = n_phi > 1 ? (phi[n_phi - 1] - phi[0]) / (n_phi - 1) : 1.0;
+    p->uniform_phi = p->dphi != 0.0;
+    for (int k = 1; k < n_phi && p->uniform_phi; ++k)
+        if (std::fabs((phi[k] - phi[k - 1]) - p->dphi) > 1e-9 * std::fabs(p->dphi)) p->uniform_phi = false;
     p->K = 1.0 / W;
     p->lambda0_sq = o.lambda0_mode == 0 ? S / W : (o.lambda0_mode == 1 ? M / n_chan : o.lambda0_sq);
 
@@ -262,7 +274,7 @@ rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
     if (!p) return RMSYNTH_OK;
     DeviceGuard guard(p->device);
     tc_plan_free(p);
-    void* ptrs[] = {p->d_delta, p->d_kw, p->d_phi, p->d_cos, p->d_sin, p->d_phif, p->d_kwf, p->d_dpi, p->d_phi2};
+    void* ptrs[] = {p->d_delta, p->d_kw, p->d_phi, p->d_cos, p->d_sin, p->d_phif, p->d_kwf, p->d_dpi, p->d_phi2, p->d_Rdw, p->d_gauss};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     for (int i = 0; i < rmsynth_plan::kScratch; ++i)
