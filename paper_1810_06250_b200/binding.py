@@ -27,7 +27,7 @@ SCHEME_AUTO, SCHEME_TF32X3, SCHEME_F16X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS 
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
            "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_execute_stream",
-           "rmsynth_rmsf", "rmsynth_rmclean",
+           "rmsynth_rmsf", "rmsynth_rmclean", "rmsynth_execute_fft",
            "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
 
 
@@ -61,6 +61,11 @@ class CleanParams(C.Structure):
     _fields_ = [("struct_size", C.c_int), ("gain", C.c_float), ("cutoff", C.c_float), ("max_iter", C.c_int), ("fwhm", C.c_float)]
 
 
+class FftParams(C.Structure):
+    _fields_ = [("struct_size", C.c_int), ("window", C.c_int), ("oversampling", C.c_float)]
+
+
+_lib.rmsynth_execute_fft.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, C.POINTER(FftParams), _vp]
 _lib.rmsynth_rmclean.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, C.POINTER(CleanParams), _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
 _lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
 _lib.rmsynth_launch_count.argtypes = [C.c_int]
@@ -169,6 +174,11 @@ class Plan:
         _check(_lib.rmsynth_execute_host(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU),
                                          _ptr(peak_amp), _ptr(peak_phi), _ptr(pa_lambda0), _ptr(pa_zero),
                                          _ptr(peak_index)))
+
+    def execute_fft(self, Q, U, n_pix, layout, FQ, FU, window=0, oversampling=0.0, stream=None):
+        """Approximate FFT variant of execute() (NEXT-4); window / oversampling 0 = defaults (6, 2)."""
+        prm = FftParams(C.sizeof(FftParams), window, oversampling)
+        _check(_lib.rmsynth_execute_fft(self._h, _ptr(Q), _ptr(U), n_pix, layout, _ptr(FQ), _ptr(FU), C.byref(prm), stream))
 
     def rmclean(self, FQ, FU, n_pix, layout, gain, cutoff, max_iter, model_q, model_u, resid_q, resid_u,
                 rest_q=None, rest_u=None, n_iter=None, fwhm=0.0, stream=None):

@@ -106,6 +106,7 @@ struct rmsynth_plan {
     mutable float gauss_fwhm = 0.f;
     mutable int gauss_reach = 0;
     mutable double rmsf_fwhm = 0.0;       // FWHM of |R| (used when the caller passes fwhm <= 0)
+    mutable void* fft_tables = nullptr;   // tables of the FFT variant for the last (window, oversampling) used (fft_variant.cu)
 };
 
 namespace rms {
@@ -121,6 +122,8 @@ rmsynth_status fp32_sincos_execute(const rmsynth_plan* p, const float* Q, const 
                                    int layout, float* FQ, float* FU, cudaStream_t st);
 // execute.cu
 void host_pipe_free(rmsynth_plan* p);
+// fft_variant.cu
+void fft_tables_free(rmsynth_plan* p);
 // peaks.cu
 rmsynth_status peaks_combine(const rmsynth_plan* p, const float* rec, int n_seg, long long n_pix, float* amp, float* phi,
                              float* pa0, float* paz, int* idx, cudaStream_t st);

@@ -282,6 +282,7 @@ rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
     for (auto& x : p->pool)
         if (x.ptr) cudaFree(x.ptr);
     host_pipe_free(p);
+    fft_tables_free(p);
     delete p;
     return RMSYNTH_OK;
 }
