@@ -142,8 +142,8 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
 
 // tc_gemm3.cu
 rmsynth_status tc3_plan_init(rmsynth_plan* p);
-rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq, bool out_phi,
-                          int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, const void* map_fq, const void* map_fu,
+                          bool a3d, bool in_freq, bool out_phi, int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
                           int sync_lag, cudaStream_t st);
 
 // tc_gemm2.cu

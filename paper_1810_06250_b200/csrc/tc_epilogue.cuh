@@ -276,24 +276,26 @@ __device__ __forceinline__ void epi_tile_phi_major_vec(const float (&acc)[128], 
     if (WITH_SCAN) sc.finish(t, lane, rec);
 }
 
-// phi-major cubes through a store warp.  One SM stores at most 32 bytes per clock (measured: 106 KB in 3.2 k cycles
-// whatever the vector width and however many SMs store), and inside this kernel, next to ~46 B/clk of inbound TMA
-// traffic, a 106 KB tile took 6.5 k cycles of the epilogue warps' time while the two TMEM accumulator buffers give
-// the MMA issuer only 2.5 k cycles of slack (profiles/r02_tile_timeline_cfg5.txt).  With few channels (few chunks per
-// tile) that stall is a large share of the item, so there the epilogue warps do not store: the four warps of a column half (128 pixels) stage a group of eight depths of FQ and of FU -- two
-// [8 depths][128 pixels] slabs, 8 KB -- in a ring of six such pairs and go back to draining accumulators; a
-// dedicated warp empties the ring with LDS.128 + st.global.cs.v4 (one instruction = one 512-byte row = four full
-// lines) and stalls on the store queue in their stead.  (TMA box stores out of the same ring were measured first:
-// ~1.7 k cycles of latency per store, so the 40 KB in flight drained at 19 B/clk.)
+// phi-major cubes through a shared-memory ring and TMA stores.  One SM stores at most 32 bytes per clock from registers
+// (measured: 106 KB in 3.2 k cycles whatever the vector width and however many SMs store), and inside this kernel, next to
+// ~46 B/clk of inbound TMA traffic, a 106 KB tile took 6.5-10 k cycles of the epilogue warps' time while the two TMEM
+// accumulator buffers give the MMA issuer only 2.5 k cycles of slack (profiles/r02_tile_timeline_cfg5_before.txt: issuer
+// blocked on acc_empty 6.6-9.5 k cycles of a 35 k-cycle item).  So the epilogue warps do not store: the four warps of a
+// column half (128 pixels) stage a group of eight depths of FQ and of FU -- two [8 depths][128 pixels] slabs, 8 KB -- in
+// a ring of ten such pairs (80 KB of the 106 KB tile: the raw-tile ring gives up its third stage for it) and go back to
+// draining accumulators; one thread of an otherwise idle warp hands every pair to the TMA engine as two box stores
+// (cp.async.bulk.tensor, 128 pixels x 8 depths; the tensor map clips ragged pixel and depth edges) and recycles a slot
+// as soon as the engine has READ it (wait_group.read).  The stores then drain in the background during the next item.
 // Pairs are used in a fixed order known to both sides: per work item, for g = 0..6: [half 0, group g] if g < ng0, then
-// [half 1, group g] if g < ng1.  full[slot]: 4 warp arrivals; empty[slot]: 1 arrival by the store warp.
-constexpr int kRingSlots = 6, kRingSlotFloats = 2048;
+// [half 1, group g] if g < ng1.  full[slot]: 4 warp arrivals; empty[slot]: 1 arrival by the store thread.
+constexpr int kRingSlots = 10, kRingSlotFloats = 2048;
 struct TileRing {
     float* base;          // kRingSlots x 2048 floats
     uint64_t* full;       // [kRingSlots]
     uint64_t* empty;      // [kRingSlots]
-    uint32_t seq;         // pairs pushed / popped so far by this thread's role (slot = seq % 6, phase = seq / 6 & 1)
-    __device__ __forceinline__ void init(float* b, uint64_t* f, uint64_t* e) { base = b; full = f; empty = e; seq = 0; }
+    uint32_t seq;         // pairs pushed / popped so far by this thread's role (slot = seq % kRingSlots, phase = seq / kRingSlots & 1)
+    uint32_t released;    // store thread only: slots handed back so far
+    __device__ __forceinline__ void init(float* b, uint64_t* f, uint64_t* e) { base = b; full = f; empty = e; seq = 0; released = 0; }
 };
 // number of 8-depth groups the two column halves hold of a depth tile with nv_tile valid depths
 __device__ __forceinline__ void ring_groups(int nv_tile, int& ng0, int& ng1) {
@@ -320,6 +322,7 @@ __device__ __forceinline__ void epi_tile_phi_major_ring(const float (&acc)[128],
                 b[e * 128 + q * 32 + lane] = acc[g * 16 + e];
                 b[1024 + e * 128 + q * 32 + lane] = acc[g * 16 + 8 + e];
             }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the TMA engine
             __syncwarp();
             if (lane == 0) mbar_arrive(&ring.full[slot]);
             if (WITH_SCAN) sc.group(acc, g, t.nv);
@@ -329,13 +332,20 @@ __device__ __forceinline__ void epi_tile_phi_major_ring(const float (&acc)[128],
     if (WITH_SCAN) sc.finish(t, lane, rec);
 }
 
-// The store warp's side: one work item = ng0 + ng1 pairs.  pix_tile: first pixel of the CTA's 128-pixel tile;
-// k_tile: first depth of the depth tile.
-__device__ __forceinline__ void ring_store_item(TileRing& ring, int lane, long long pix_tile, int k_tile, int nv_tile, long long n_pix,
-                                                float* __restrict__ FQ, float* __restrict__ FU) {
+// The store thread's side: one work item = ng0 + ng1 pairs.  pix_tile: first pixel of the CTA's 128-pixel tile;
+// k_tile: first depth of the depth tile.  Called by ONE thread.
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int c0, int c1, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;" ::"l"(map), "r"(src),
+                 "r"(c0), "r"(c1), "l"(pol) : "memory");
+}
+constexpr int kRingPending = 6;   // bulk groups that may still be reading their slot when the store thread moves on
+__device__ __forceinline__ void ring_release(TileRing& ring, uint32_t upto) {      // slots of the groups < upto go back
+    for (; ring.released < upto; ++ring.released) mbar_arrive(&ring.empty[ring.released % kRingSlots]);
+}
+__device__ __forceinline__ void ring_store_item(TileRing& ring, const CUtensorMap* mapFQ, const CUtensorMap* mapFU, int pix_tile,
+                                                int k_tile, int nv_tile, uint64_t pol) {
     int ng0, ng1;
     ring_groups(nv_tile, ng0, ng1);
-    const bool pin = pix_tile + lane * 4 < n_pix;                // n_pix % 4 == 0: four pixels in range or none
     for (int g = 0; g < 7; ++g) {
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
@@ -343,33 +353,20 @@ __device__ __forceinline__ void ring_store_item(TileRing& ring, int lane, long l
             const uint32_t slot = ring.seq % kRingSlots, phase = (ring.seq / kRingSlots) & 1u;
             ++ring.seq;
             mbar_wait(&ring.full[slot], phase);
-            const float4* b = reinterpret_cast<const float4*>(ring.base + slot * kRingSlotFloats) + lane;
-            const int d0 = half * 56 + g * 8;                    // first local depth of the pair
-            const long long row = (long long)(k_tile + d0) * n_pix + pix_tile + lane * 4;
-#pragma unroll
-            for (int h = 0; h < 4; ++h) {                        // two depth rows of both cubes per round (the warp has 32 registers)
-                float4 vq[2], vu[2];
-#pragma unroll
-                for (int i = 0; i < 2; ++i) { vq[i] = b[(h * 2 + i) * 32]; vu[i] = b[256 + (h * 2 + i) * 32]; }
-                if (h == 3) {
-                    // the slot goes back as soon as its last rows have ARRIVED in registers (the dummy AND makes the
-                    // arrival wait for them), not when the stores below have found room in the store queue
-                    uint32_t z0, z1;
-                    asm volatile("and.b32 %0, %1, 0;" : "=r"(z0) : "r"(__float_as_uint(vq[1].w)));
-                    asm volatile("and.b32 %0, %1, 0;" : "=r"(z1) : "r"(__float_as_uint(vu[1].w)));
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&ring.empty[slot + z0 + z1]);
-                }
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    if (pin && d0 + h * 2 + i < nv_tile) {
-                        __stcs(reinterpret_cast<float4*>(FQ + row + (h * 2 + i) * n_pix), vq[i]);
-                        __stcs(reinterpret_cast<float4*>(FU + row + (h * 2 + i) * n_pix), vu[i]);
-                    }
-                }
-            }
+            const uint32_t src = smem_u32(ring.base + slot * kRingSlotFloats);
+            const int d0 = k_tile + half * 56 + g * 8;           // first depth of the pair
+            tma_store_2d(mapFQ, src, pix_tile, d0, pol);
+            tma_store_2d(mapFU, src + 4096, pix_tile, d0, pol);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kRingPending) : "memory");
+            if (ring.seq > (uint32_t)kRingPending) ring_release(ring, ring.seq - kRingPending);
         }
     }
+    // nothing else to do until the next tile end: wait until the engine has read the item's last slots, hand them all back
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    ring_release(ring, ring.seq);
 }
+// before the kernel exits: every bulk store has been performed (written), not merely read
+__device__ __forceinline__ void ring_store_flush() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 }  // namespace rms

@@ -167,21 +167,23 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     if (gang < 1 || gang > T || T % gang) gang = T;
     if (gang > p->sm_count / 2) gang = 1;                    // more depth tiles than CTA pairs: every cluster on its own
     if (sync_lag < 0 || gang == 1) tile_sync = nullptr;
-    // Tile end of the FP16 kernel for phi-major cubes (tc_epilogue.cuh).  One SM stores 32 B/clk at most, so a 106 KB tile
-    // is >= 3.3 k cycles of store-port time against 2.5 k cycles of accumulator slack: with few channels per tile
-    // (<= 16 chunks of 32) the tile goes through a shared-memory ring and a store warp (1), with more the epilogue warps
-    // store it themselves with 8-byte vectors (2: the stall is a small share of a long item and the ring's extra
-    // shared-memory traffic costs more, measured 2.94 vs 3.2 ms on configs[1]); odd shapes take the scalar path (0).
-    // With 1 and 2 the peak search records only (max |F|^2, k) per segment and peaks_gather_kernel reads the three
-    // samples around k* back from the cubes.
+    // Tile end of the FP16 kernel for phi-major cubes (tc_epilogue.cuh).  One SM stores 32 B/clk at most from registers, so a
+    // 106 KB tile is >= 3.3 k cycles of store-port time against 2.5 k cycles of accumulator slack: the tile goes through a
+    // shared-memory ring and TMA box stores (1) whenever TMA can address the cubes (16-byte aligned rows); else the epilogue
+    // warps store it themselves with 8-byte vectors (2) or scalars (0).  With 1 and 2 the peak search records only
+    // (max |F|^2, k) per segment and peaks_gather_kernel reads the three samples around k* back from the cubes.
     int ring_out = 0;
+    CUtensorMap mfq, mfu;
     if (f16 && out_phi && FQ && !FA && !getenv("RMSYNTH_NO_RING_OUT")) {
-        const int n_chunks = p->tc3.k_pad / p->tc3.kb;
-        const char* force = getenv("RMSYNTH_RING_OUT");      // EXPERIMENT knob
-        if (n_pix % 4 == 0 && !((uintptr_t)FQ & 15) && !((uintptr_t)FU & 15) && (force ? atoi(force) == 1 : n_chunks <= 16)) ring_out = 1;
+        const char* force = getenv("RMSYNTH_RING_OUT");      // EXPERIMENT knob: 1 = ring + TMA stores, 2 = vector stores
+        const int want = force ? atoi(force) : 1;
+        if (want == 1 && n_pix % 4 == 0 && n_pix < (1LL << 31) && !((uintptr_t)FQ & 15) && !((uintptr_t)FU & 15)) ring_out = 1;
         else if (n_pix % 2 == 0 && !((uintptr_t)FQ & 7) && !((uintptr_t)FU & 7)) ring_out = 2;
+        if (ring_out == 1 && ((s = make_map(&mfq, FQ, n_pix, p->n_phi, n_pix, 128, 8, CU_TENSOR_MAP_SWIZZLE_NONE)) ||
+                              (s = make_map(&mfu, FU, n_pix, p->n_phi, n_pix, 128, 8, CU_TENSOR_MAP_SWIZZLE_NONE))))
+            return s;
     }
-    s = f16 ? tc3_launch(p, &mq, &mu_, a3d, in_freq, out_phi, ring_out, n_pix, FQ, FU, FA, rec, tile_sync, gang, sync_lag, st)
+    s = f16 ? tc3_launch(p, &mq, &mu_, &mfq, &mfu, a3d, in_freq, out_phi, ring_out, n_pix, FQ, FU, FA, rec, tile_sync, gang, sync_lag, st)
             : tc2_launch(p, &mq, &mu_, a3d, in_freq, out_phi, n_pix, FQ, FU, FA, rec, tile_sync, gang, sync_lag, st);
     if (s) return s;
     if (!want_maps) return RMSYNTH_OK;

@@ -42,20 +42,30 @@ constexpr int T3_NMAX = 104;                     // depths per tile: 2 x 2n accu
 constexpr int T3_KC = 32;                        // channels per chunk (scale and drain granularity)
 constexpr int T3_RAW = 2 * T3_M * T3_KC * 4;     // 32 KB: raw Q tile + raw U tile of one chunk
 constexpr int T3_BSTAGE = 256 * T3_NMAX;         // 26 KB: [hi|lo][slot0|slot1][4 k-cores][n rows][8 halves]
-constexpr int T3_R = 3, T3_S = 3, T3_NA = 3;     // raw ring, B ring (chunks); A ring in TMEM (16-channel slots)
+constexpr int T3_S = 3, T3_NA = 3;               // B ring (chunks); A ring in TMEM (16-channel slots)
 constexpr int T3_SCALES = 8;                     // ring of per-pixel chunk scales (transform -> epilogue)
 constexpr int T3_ACC_COLS = 208, T3_A_COL0 = 416;
-constexpr int T3_OFF_B = T3_R * T3_RAW;
-constexpr int T3_OFF_SCALE = T3_OFF_B + T3_S * T3_BSTAGE;
-constexpr int T3_OFF_BARS = T3_OFF_SCALE + T3_SCALES * T3_M * 2;   // scales are powers of two: kept as bf16 bit patterns
 constexpr int T3_MASKS = 48;                     // channel masks of the first 48 chunks live in shared memory
-constexpr int T3_OFF_MASK = T3_OFF_BARS + 320;   // 34 barriers + the TMEM address word come first
-constexpr int T3_OFF_STAGE_T = T3_OFF_BARS + 512;
-constexpr int T3_SMEM_PHI = T3_OFF_STAGE_T + kRingSlots * 8192 + 1024; // output ring (6 pairs x 8 KB) + alignment slack
-static_assert(T3_SMEM_PHI <= 227 * 1024, "shared memory budget");
-constexpr int T3_SMEM_LOS = T3_OFF_STAGE_T + 8 * 32 * 33 * 4 + 1024;
 constexpr int T3_THREADS = 512;
-static_assert(T3_SMEM_LOS <= 227 * 1024, "shared memory budget");
+// Shared-memory layout.  The raw ring has three stages, except in the ring-output variant (OUT == 2), where the third
+// stage's 32 KB go to the output ring: a raw stage is held only from the TMA landing to the transform's read at the
+// start of its chunk, so with two stages a load still has two chunk periods (~4 k cycles) to arrive.
+template <int OUT>
+struct T3Lay {
+    static constexpr int R = OUT == 2 ? 2 : 3;                        // raw ring stages (chunks)
+    static constexpr int OFF_B = R * T3_RAW;
+    static constexpr int OFF_SCALE = OFF_B + T3_S * T3_BSTAGE;
+    static constexpr int OFF_BARS = OFF_SCALE + T3_SCALES * T3_M * 2;  // scales are powers of two: kept as bf16 bit patterns
+    static constexpr int OFF_MASK = OFF_BARS + 384;                    // <= 44 barriers + the TMEM address word come first
+    static constexpr int OFF_STAGE = OFF_BARS + 640;                   // 128-byte aligned (TMA store source)
+    static constexpr int STAGE_BYTES = OUT == 2 ? kRingSlots * 8192    // output ring (ten pairs x 8 KB)
+                                     : OUT == 1 ? 8 * 32 * 33 * 4      // LOS-major transpose buffers
+                                     : OUT == 3 ? 8 * 1024 * 4 : 0;    // per-warp turn-around buffers of the vectorised stores
+    static constexpr int SMEM = OFF_STAGE + STAGE_BYTES + 1024;        // + alignment slack
+    static_assert(OFF_STAGE % 128 == 0, "stage alignment");
+    static_assert(2 * T3_S + 2 * T3_NA + 4 + 2 * 3 + 2 * kRingSlots <= 48, "barrier area");
+    static_assert(SMEM <= 227 * 1024, "shared memory budget");
+};
 
 __device__ __forceinline__ void umma2_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
     asm volatile(
@@ -189,13 +199,16 @@ __device__ __forceinline__ void t3_accumulate(uint64_t* acc2, const uint32_t* r,
 //      2 = phi-major through the output ring and the store warp, 3 = phi-major, vectorised stores (tc_epilogue.cuh)
 template <int IN_MN, int OUT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
-tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU, const Tc3Params prm) {
+tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU,
+                   const __grid_constant__ CUtensorMap mapFQ, const __grid_constant__ CUtensorMap mapFU, const Tc3Params prm) {
     constexpr bool OUT_LOS = OUT == 1;
+    using L = T3Lay<OUT>;
+    constexpr int T3_R = L::R;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    uint16_t* scales = reinterpret_cast<uint16_t*>(smem_gen + T3_OFF_SCALE);      // [T3_SCALES][128] upper halves of FP32 powers of two
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_gen + T3_OFF_BARS);
+    uint16_t* scales = reinterpret_cast<uint16_t*>(smem_gen + L::OFF_SCALE);      // [T3_SCALES][128] upper halves of FP32 powers of two
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_gen + L::OFF_BARS);
     uint64_t* raw_full = bars;                    // [R] raw tile landed                     (1 + tx)
     uint64_t* raw_empty = raw_full + T3_R;        // [R] raw tile read by the transform      (4 warps)
     uint64_t* b_full = raw_empty + T3_R;          // [S] B chunk landed                      (1 + tx)
@@ -204,11 +217,11 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     uint64_t* a_empty = a_ready + T3_NA;          // [NA] MMAs that read the slot done        (multicast commit)
     uint64_t* acc_full = a_empty + T3_NA;         // [2] chunk accumulated, both CTAs         (multicast commit)
     uint64_t* acc_empty = acc_full + 2;           // [2] LEADER's: chunk drained by both epilogues (8 + 8 warps)
-    uint64_t* ring_full = acc_empty + 2;          // [6] output pair staged                           (4 epilogue warps)
-    uint64_t* ring_empty = ring_full + kRingSlots; // [6] output pair read by the store warp          (1)
+    uint64_t* ring_full = acc_empty + 2;          // [10] output pair staged                          (4 epilogue warps)
+    uint64_t* ring_empty = ring_full + kRingSlots; // [10] output pair read by the TMA engine          (store thread)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ring_empty + kRingSlots);
-    uint32_t* smask = reinterpret_cast<uint32_t*>(smem_gen + T3_OFF_MASK);        // [T3_MASKS]
-    float* stage_t = reinterpret_cast<float*>(smem_gen + T3_OFF_STAGE_T);         // LOS-major transpose buffers
+    uint32_t* smask = reinterpret_cast<uint32_t*>(smem_gen + L::OFF_MASK);        // [T3_MASKS]
+    float* stage_t = reinterpret_cast<float*>(smem_gen + L::OFF_STAGE);         // LOS-major transpose buffers
 
     // warp index through a shuffle: provably warp-uniform, so role branches are uniform and MMA operands stay in uniform registers
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
@@ -306,7 +319,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&b_empty[st], ph ^ 1);
                     mbar_expect_tx(&b_full[st], b_bytes);
-                    bulk_load(smem_base + T3_OFF_B + st * T3_BSTAGE, bsrc + (size_t)c * 2 * b_bytes, b_bytes, &b_full[st], pol);
+                    bulk_load(smem_base + L::OFF_B + st * T3_BSTAGE, bsrc + (size_t)c * 2 * b_bytes, b_bytes, &b_full[st], pol);
                     if (++st == T3_S) { st = 0; ph ^= 1; }
                 }
             }
@@ -340,7 +353,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     tl.add(c < 2 ? 4 : 1);                 // slot 4: the first two chunks of an item (the tile-end bubble)
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_u + ab * T3_ACC_COLS;
-                    const uint32_t baddr = (smem_u + T3_OFF_B + sb * T3_BSTAGE) >> 4;
+                    const uint32_t baddr = (smem_u + L::OFF_B + sb * T3_BSTAGE) >> 4;
 #pragma unroll
                     for (int ks = 0; ks < 2; ++ks) {
                         tl.begin();
@@ -372,14 +385,19 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
         __syncwarp();
       } else if (OUT == 2) {
-        // ===================== store warp (both CTAs): output ring -> global (tc_epilogue.cuh) =====================
-        TileRing ring;
-        ring.init(stage_t, ring_full, ring_empty);
-        WorkIter wi;
-        wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
-        int tp, j;
-        while (wi.next(tp, j))
-            ring_store_item(ring, lane, (long long)(2 * tp + (int)rank) * T3_M, j * n, min(n, prm.n_phi - j * n), prm.n_pix, prm.FQ, prm.FU);
+        // ===================== store thread (both CTAs): output ring -> TMA box stores (tc_epilogue.cuh) =====================
+        if (lane == 0) {
+            const uint64_t pol = l2_policy_evict_first();
+            TileRing ring;
+            ring.init(stage_t, ring_full, ring_empty);
+            WorkIter wi;
+            wi.init(cluster_id, n_clusters, prm.n_phi_tiles, prm.n_pairs, prm.gang);
+            int tp, j;
+            while (wi.next(tp, j))
+                ring_store_item(ring, &mapFQ, &mapFU, (2 * tp + (int)rank) * T3_M, j * n, min(n, prm.n_phi - j * n), pol);
+            ring_store_flush();
+        }
+        __syncwarp();
       }
     } else if (warp >= 12) {
         // ===================== transform (both CTAs): raw FP32 tile -> scaled FP16 hi/lo in TMEM =====================
@@ -603,14 +621,14 @@ rmsynth_status tc3_plan_init(rmsynth_plan* p) {
                                      std::ldexp(1.0, p->tc3_eb), reinterpret_cast<__half*>(p->d_tcB3));
     RMS_LAUNCH_CHECK("tc3_build_b_kernel");
 #define T3_ATTR(IN, O, BYTES) RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<IN, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES))
-    T3_ATTR(0, 0, T3_SMEM_PHI); T3_ATTR(1, 0, T3_SMEM_PHI); T3_ATTR(0, 1, T3_SMEM_LOS); T3_ATTR(1, 1, T3_SMEM_LOS);
-    T3_ATTR(0, 2, T3_SMEM_PHI); T3_ATTR(1, 2, T3_SMEM_PHI); T3_ATTR(0, 3, T3_SMEM_PHI); T3_ATTR(1, 3, T3_SMEM_PHI);
+    T3_ATTR(0, 0, T3Lay<0>::SMEM); T3_ATTR(1, 0, T3Lay<0>::SMEM); T3_ATTR(0, 1, T3Lay<1>::SMEM); T3_ATTR(1, 1, T3Lay<1>::SMEM);
+    T3_ATTR(0, 2, T3Lay<2>::SMEM); T3_ATTR(1, 2, T3Lay<2>::SMEM); T3_ATTR(0, 3, T3Lay<3>::SMEM); T3_ATTR(1, 3, T3Lay<3>::SMEM);
 #undef T3_ATTR
     return RMSYNTH_OK;
 }
 
-rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, bool a3d, bool in_freq, bool out_phi,
-                          int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
+rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* map_u, const void* map_fq, const void* map_fu,
+                          bool a3d, bool in_freq, bool out_phi, int ring_out, long long n_pix, float* FQ, float* FU, float* FA, float* rec, int* tile_sync, int gang,
                           int sync_lag, cudaStream_t st) {
     Tc3Params prm;
     prm.n_pix = n_pix;
@@ -653,8 +671,10 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     const CUtensorMap& mq = *static_cast<const CUtensorMap*>(map_q);
     const CUtensorMap& mu = *static_cast<const CUtensorMap*>(map_u);
     const int out = !out_phi ? 1 : ring_out == 1 ? 2 : ring_out == 2 ? 3 : 0;
-    const int smem = out == 1 ? T3_SMEM_LOS : T3_SMEM_PHI;
-#define T3_LAUNCH(IN, O) tc3_rmsynth_kernel<IN, O><<<grid, T3_THREADS, smem, st>>>(mq, mu, prm)
+    // output tensor maps are read by the ring variant only; the others get the input maps as placeholders
+    const CUtensorMap& mfq = *static_cast<const CUtensorMap*>(out == 2 ? map_fq : map_q);
+    const CUtensorMap& mfu = *static_cast<const CUtensorMap*>(out == 2 ? map_fu : map_u);
+#define T3_LAUNCH(IN, O) tc3_rmsynth_kernel<IN, O><<<grid, T3_THREADS, T3Lay<O>::SMEM, st>>>(mq, mu, mfq, mfu, prm)
     switch (out * 2 + (in_freq ? 1 : 0)) {
         case 0: T3_LAUNCH(0, 0); break;
         case 1: T3_LAUNCH(1, 0); break;
