@@ -56,8 +56,7 @@ enum {
     RMSYNTH_SCHEME_TF32X3 = 1,      /* tcgen05 tensor cores, split-precision 3xTF32,     */
                                     /* FP32 accumulate in TMEM                           */
     RMSYNTH_SCHEME_F16X3 = 2,       /* tcgen05 tensor cores, block-scaled FP16 hi/lo split    */
-                                    /* (3 products at twice the TF32 rate), FP32 accumulate;  */
-                                    /* zero-weight channels are ignored even if non-finite    */
+                                    /* (3 products at twice the TF32 rate), FP32 accumulate   */
     RMSYNTH_SCHEME_FP32_TABLE = 3,  /* CUDA cores, FP32 FMA, reads the plan's cos/sin    */
     RMSYNTH_SCHEME_FP32_SINCOS = 4  /* CUDA cores, sincos on the fly, one (pixel,phi)    */
                                     /* per thread -- the paper's kernel shape    */
@@ -101,11 +100,16 @@ rmsynth_status rmsynth_plan_phase_matrix(const rmsynth_plan *plan, float *cos_kw
 /* Eqs. 15-16 for n_pix lines of sight.
  *   Q, U    DEVICE, n_pix*n_chan floats each, input layout per `layout`
  *   FQ, FU  DEVICE, n_pix*n_phi floats each, output layout per `layout`
- *   stream  a cudaStream_t (NULL = default stream).  The call only enqueues work; it never
- *           synchronises and never allocates after the plan's first use on a shape.
+ *   stream  a cudaStream_t (NULL = default stream).  The call only enqueues work and never
+ *           synchronises.  Per-stream workspace (peak records, check-in counters) is allocated
+ *           on the first call of a (stream, size) and only ever grows; outgrown buffers stay
+ *           alive until rmsynth_plan_destroy, so a CUDA graph captured from an earlier call
+ *           remains valid.  Inside a stream capture the workspace cannot grow (EINVAL): run
+ *           the shape once on that stream before capturing.
  * n_pix == 0 is a successful no-op.  EINVAL: n_pix < 0, NULL Q/U/FQ/FU, unknown layout bits.
- * Non-finite samples propagate to the outputs of their pixel (no masking); the F16X3 scheme
- * alone ignores the samples of zero-weight channels altogether, non-finite or not. */
+ * Non-finite samples propagate to the outputs of their pixel (its cubes are NaN, its maps NaN
+ * with peak_index -1).  Channels with w_i = 0 are REMOVED (reading A13): every scheme ignores
+ * their samples altogether, non-finite or not -- a NaN-blanked flagged plane does no harm. */
 rmsynth_status rmsynth_execute(const rmsynth_plan *plan, const float *Q, const float *U,
                                long long n_pix, int layout, float *FQ, float *FU, void *stream);
 

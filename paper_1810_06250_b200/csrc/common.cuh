@@ -96,6 +96,7 @@ struct rmsynth_plan {
     struct StreamScratch { cudaStream_t st; int tag; float* ptr; size_t bytes; };
     mutable std::mutex pool_mu;
     mutable std::vector<StreamScratch> pool;
+    mutable std::vector<float*> retired;  // outgrown workspace buffers, kept until destroy (captured graphs may reference them)
     mutable void* host_pipe = nullptr;    // streams, events and staging of the host-streaming engine (execute.cu)
     long long host_chunk_pixels = 0;      // rmsynth_options.host_chunk_pixels (0 = automatic)
     // RM-CLEAN (rmclean.cu): needs a uniform depth grid; beam and restoring Gaussian are built on first use

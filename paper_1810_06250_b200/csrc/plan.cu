@@ -42,8 +42,13 @@ rmsynth_status stream_scratch(const rmsynth_plan* p, cudaStream_t st, int tag, s
         e = &p->pool.back();
     }
     if (e->bytes < bytes) {
-        // the old buffer may still be in use by work already enqueued on this stream
-        if (e->ptr) { RMS_CUDA(cudaStreamSynchronize(st)); cudaFree(e->ptr); }
+        // Growing never frees: work already enqueued on this stream, or a CUDA graph captured from an earlier call, may
+        // still reference the old buffer, so it is retired and lives until the plan is destroyed.  An allocation cannot
+        // happen inside a stream capture: the caller must run the shape once (or a larger one) before capturing.
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
+            return fail(RMSYNTH_EINVAL, "workspace must grow during a stream capture: execute this shape once before capturing");
+        if (e->ptr) p->retired.push_back(e->ptr);
         e->ptr = nullptr;
         e->bytes = 0;
         RMS_CUDA(cudaMalloc(&e->ptr, bytes));
@@ -281,6 +286,7 @@ rmsynth_status rmsynth_plan_destroy(rmsynth_plan* p) {
         if (p->scratch[i]) cudaFree(p->scratch[i]);
     for (auto& x : p->pool)
         if (x.ptr) cudaFree(x.ptr);
+    for (float* q : p->retired) cudaFree(q);
     host_pipe_free(p);
     fft_tables_free(p);
     delete p;

@@ -31,6 +31,7 @@
 #include <cuda_fp16.h>
 #include <cstdio>
 #include <cstdlib>
+#include <type_traits>
 #include "common.cuh"
 #include "tc_common.cuh"
 #include "tc_epilogue.cuh"
@@ -196,8 +197,11 @@ __device__ __forceinline__ void t3_accumulate(uint64_t* acc2, const uint32_t* r,
 }
 
 // OUT: 0 = phi-major cubes, scalar stores (any shape; also |F| cube and maps-only calls), 1 = LOS-major cubes,
-//      2 = phi-major through the output ring and the store warp, 3 = phi-major, vectorised stores (tc_epilogue.cuh)
-template <int IN_MN, int OUT>
+//      2 = phi-major through the output ring and TMA stores, 3 = phi-major, vectorised stores (tc_epilogue.cuh)
+// TAIL: the last chunk holds at most 16 real channels (0 < n_chan % 32 <= 16): its second, all-zero K step is neither
+//      transformed nor multiplied (configs[4]: 400 channels = 12.5 chunks -> 6 of 156 MMAs per work item).  A separate
+//      instantiation with the last chunk peeled off the loop, so the other shapes do not pay a branch per chunk.
+template <int IN_MN, int OUT, bool TAIL>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
 tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapU,
                    const __grid_constant__ CUtensorMap mapFQ, const __grid_constant__ CUtensorMap mapFU, const Tc3Params prm) {
@@ -230,6 +234,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const int n = prm.n, N2 = 2 * prm.n;
     const uint32_t b_bytes = 256u * n;
     const int n_chunks = prm.n_chunks;
+    const int n_full = TAIL ? n_chunks - 1 : n_chunks;      // chunks with two K steps
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < T3_R; ++s) { mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], 4); }
@@ -347,7 +352,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             int tp, j;
             while (wi.next(tp, j)) {
                 tl.stamp(0);
-                for (int c = 0; c < n_chunks; ++c) {
+                auto chunk = [&](int c, auto two_steps) {
                     tl.begin();
                     mbar_wait(&acc_empty[ab], aph ^ 1);
                     tl.add(c < 2 ? 4 : 1);                 // slot 4: the first two chunks of an item (the tile-end bubble)
@@ -355,7 +360,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     const uint32_t d_tmem = tmem_u + ab * T3_ACC_COLS;
                     const uint32_t baddr = (smem_u + L::OFF_B + sb * T3_BSTAGE) >> 4;
 #pragma unroll
-                    for (int ks = 0; ks < 2; ++ks) {
+                    for (int ks = 0; ks < (decltype(two_steps)::value ? 2 : 1); ++ks) {
                         tl.begin();
                         mbar_wait(&a_ready[sa], pa);       // A slot written and (ks == 0) B chunk landed, in both CTAs
                         tl.add(c == 0 && ks == 0 ? 5 : 2); // slot 5: the first A slot of an item
@@ -378,7 +383,9 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                     __syncwarp();
                     if (++sb == T3_S) sb = 0;
                     if (++ab == 2) { ab = 0; aph ^= 1; }
-                }
+                };
+                for (int c = 0; c < n_full; ++c) chunk(c, std::true_type());
+                if (TAIL) chunk(n_full, std::false_type());
                 tl.stamp(3);
                 tl.next();
             }
@@ -415,7 +422,8 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         int tp, j;
         while (wi.next(tp, j)) {
             tl.stamp(0);
-            for (int c = 0; c < n_chunks; ++c) {
+            auto chunk = [&](int c, auto two_steps) {
+                constexpr bool TWO = decltype(two_steps)::value;    // false: the half-filled last chunk (TAIL), one 16-channel slot
                 float v[64];
                 tl.begin();
                 mbar_wait(&raw_full[sr], pr);
@@ -462,10 +470,12 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 tl.lap(2);
                 tc_fence_after();
                 tmem_st32(tmem + lane_addr + T3_A_COL0 + s0 * 32, r0);
+                if (TWO) {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {                        // the second conversion overlaps the first store
-                    t3_split(v[16 + 2 * i], v[16 + 2 * i + 1], scale2, r1[i], r1[8 + i]);
-                    t3_split(v[48 + 2 * i], v[48 + 2 * i + 1], scale2, r1[16 + i], r1[24 + i]);
+                    for (int i = 0; i < 8; ++i) {                    // the second conversion overlaps the first store
+                        t3_split(v[16 + 2 * i], v[16 + 2 * i + 1], scale2, r1[i], r1[8 + i]);
+                        t3_split(v[48 + 2 * i], v[48 + 2 * i + 1], scale2, r1[16 + i], r1[24 + i]);
+                    }
                 }
                 tl.lap(6);
                 tmem_st_wait();
@@ -476,6 +486,7 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(ready0 + s0 * 8);
+                if (!TWO) { sa = s1; pa = p1; return; }
                 mbar_wait(&a_empty[s1], p1 ^ 1);
                 tl.lap(2);
                 tc_fence_after();
@@ -488,7 +499,9 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 pa = p1;
                 sa = s1 + 1 == T3_NA ? 0 : s1 + 1;
                 if (sa == 0) pa ^= 1;
-            }
+            };
+            for (int c = 0; c < n_full; ++c) chunk(c, std::true_type());
+            if (TAIL) chunk(n_full, std::false_type());
             tl.stamp(4);
             tl.next();
         }
@@ -620,7 +633,9 @@ rmsynth_status tc3_plan_init(rmsynth_plan* p) {
     tc3_build_b_kernel<<<grid, 64>>>(p->d_delta, p->d_kw, p->d_phi, p->n_chan, p->n_phi, g.n_tile, n_chunks,
                                      std::ldexp(1.0, p->tc3_eb), reinterpret_cast<__half*>(p->d_tcB3));
     RMS_LAUNCH_CHECK("tc3_build_b_kernel");
-#define T3_ATTR(IN, O, BYTES) RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<IN, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES))
+#define T3_ATTR(IN, O, BYTES)                                                                                                        \
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<IN, O, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES)); \
+    RMS_CUDA(cudaFuncSetAttribute(tc3_rmsynth_kernel<IN, O, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, BYTES))
     T3_ATTR(0, 0, T3Lay<0>::SMEM); T3_ATTR(1, 0, T3Lay<0>::SMEM); T3_ATTR(0, 1, T3Lay<1>::SMEM); T3_ATTR(1, 1, T3Lay<1>::SMEM);
     T3_ATTR(0, 2, T3Lay<2>::SMEM); T3_ATTR(1, 2, T3Lay<2>::SMEM); T3_ATTR(0, 3, T3Lay<3>::SMEM); T3_ATTR(1, 3, T3Lay<3>::SMEM);
 #undef T3_ATTR
@@ -674,7 +689,10 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     // output tensor maps are read by the ring variant only; the others get the input maps as placeholders
     const CUtensorMap& mfq = *static_cast<const CUtensorMap*>(out == 2 ? map_fq : map_q);
     const CUtensorMap& mfu = *static_cast<const CUtensorMap*>(out == 2 ? map_fu : map_u);
-#define T3_LAUNCH(IN, O) tc3_rmsynth_kernel<IN, O><<<grid, T3_THREADS, T3Lay<O>::SMEM, st>>>(mq, mu, mfq, mfu, prm)
+    const bool tail = p->n_chan % T3_KC != 0 && p->n_chan % T3_KC <= T3_KC / 2;   // the last chunk's second K step is all padding
+#define T3_LAUNCH(IN, O)                                                                                   \
+    if (tail) tc3_rmsynth_kernel<IN, O, true><<<grid, T3_THREADS, T3Lay<O>::SMEM, st>>>(mq, mu, mfq, mfu, prm); \
+    else tc3_rmsynth_kernel<IN, O, false><<<grid, T3_THREADS, T3Lay<O>::SMEM, st>>>(mq, mu, mfq, mfu, prm)
     switch (out * 2 + (in_freq ? 1 : 0)) {
         case 0: T3_LAUNCH(0, 0); break;
         case 1: T3_LAUNCH(1, 0); break;
