@@ -110,23 +110,34 @@ __global__ void __launch_bounds__(256) peaks_gather_kernel(
     if (p >= n_pix) return;
     PeakState s;
     s.init();
-    for (int g = 0; g < n_seg; ++g) {
-        const float* r = rec + (long long)g * kPeakFields * n_pix + p;
-        const float by2 = r[0];
-        s.nonfinite += by2 * 0.f;
-        if (by2 > s.best_y2) { s.best_y2 = by2; s.best_k = __float_as_int(r[1 * n_pix]); }
+    // Two memory round trips per pixel, not n_seg + 1: the segment records are fetched eight at a time with
+    // unconditional, independent loads (a load of k guarded by the comparison would chain the segments), then the three
+    // samples around k* with clamped indices.
+    for (int g0 = 0; g0 < n_seg; g0 += 8) {
+        float y[8];
+        int kk[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const bool ok = g0 + i < n_seg;
+            const float* r = rec + (long long)(ok ? g0 + i : g0) * kPeakFields * n_pix + p;
+            const float v = __ldcs(r);
+            kk[i] = __float_as_int(__ldcs(r + n_pix));
+            y[i] = ok ? v : -2.f;                              // a padding slot never wins and is finite
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            s.nonfinite += y[i] * 0.f;
+            if (y[i] > s.best_y2) { s.best_y2 = y[i]; s.best_k = kk[i]; }
+        }
     }
-    const int k = s.best_k;
-    auto y2_at = [&](int kk, float& q, float& u) {
-        const size_t i = out_phi ? (size_t)kk * n_pix + p : (size_t)p * n_phi + kk;
-        q = FQ[i];
-        u = FU[i];
-        return fmaf(q, q, u * u);
-    };
-    float q, u;
-    s.best_y2 = y2_at(k, s.best_q, s.best_u);
-    if (k > 0) s.best_ym2 = y2_at(k - 1, q, u);
-    if (k < n_phi - 1) s.best_yp2 = y2_at(k + 1, q, u);
+    const int k = s.best_k, km = max(k - 1, 0), kp = min(k + 1, n_phi - 1);
+    auto at = [&](int kk) { return out_phi ? (size_t)kk * n_pix + p : (size_t)p * n_phi + kk; };
+    const float q0 = FQ[at(k)], u0 = FU[at(k)], qm = FQ[at(km)], um = FU[at(km)], qp = FQ[at(kp)], up = FU[at(kp)];
+    s.best_q = q0;
+    s.best_u = u0;
+    s.best_y2 = fmaf(q0, q0, u0 * u0);
+    if (k > 0) s.best_ym2 = fmaf(qm, qm, um * um);
+    if (k < n_phi - 1) s.best_yp2 = fmaf(qp, qp, up * up);
     refine_and_store(s, n_phi, phif, lambda0_sq, p, amp, phi, pa0, paz, idx);
 }
 
