@@ -86,7 +86,6 @@ struct rmsynth_plan {
     void* d_tcB3 = nullptr;               // scaled FP16 hi/lo B operand blobs
     unsigned int* d_chanmask = nullptr;   // per 32 channels: bit i set = channel exists and has w > 0 (reading A13)
     int tc3_eb = 0;                       // B is scaled by 2^tc3_eb
-    void* tc_maps = nullptr;              // host-side CUtensorMap cache
     // scratch for maps-only calls and host streaming (grown on demand, guarded by mu)
     mutable std::mutex mu;
     static constexpr int kScratch = 15;   // host-streaming slots: (Q, U, FQ, FU, maps) x 3

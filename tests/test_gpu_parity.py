@@ -498,7 +498,42 @@ def test_execute_is_capturable_in_a_cuda_graph(b, oracle_mod):
         torch.cuda.synchronize()
         check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, f"graph replay {scheme}")
         assert int(idx.min()) >= 0
+        # The workspace rule of rmsynth.h: a larger call on the same stream makes the workspace grow, which must not
+        # invalidate the captured graph (outgrown buffers live until the plan is destroyed) ...
+        big = 4 * 640
+        cfg2, _, _, _, q2, u2 = inputs(1, big)
+        dq2, du2 = torch.from_numpy(q2).cuda(), torch.from_numpy(u2).cuda()
+        fq2 = torch.zeros(big, plan.n_phi, device="cuda")
+        fu2 = torch.zeros_like(fq2)
+        idx2 = torch.zeros(big, dtype=torch.int32, device="cuda")
+        with torch.cuda.stream(s):
+            plan.execute_peaks(dq2, du2, big, 0, fq2, fu2, peak_index=idx2, stream=s.cuda_stream)
+        s.synchronize()
+        fq.fill_(float("nan"))
+        fu.fill_(float("nan"))
+        idx.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, f"graph replay after workspace growth {scheme}")
+        assert int(idx.min()) >= 0
         del g
+        # ... and inside a capture the workspace cannot grow: EINVAL, nothing enqueued, the capture stays usable
+        bigger = 8 * 640
+        cfg3, _, _, _, q3, u3 = inputs(1, bigger)
+        dq3, du3 = torch.from_numpy(q3).cuda(), torch.from_numpy(u3).cuda()
+        fq3 = torch.zeros(bigger, plan.n_phi, device="cuda")
+        fu3 = torch.zeros_like(fq3)
+        idx3 = torch.zeros(bigger, dtype=torch.int32, device="cuda")
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=s):
+            with pytest.raises(b.RmsynthError) as e:
+                plan.execute_peaks(dq3, du3, bigger, 0, fq3, fu3, peak_index=idx3, stream=torch.cuda.current_stream().cuda_stream)
+            assert e.value.status == b.EINVAL
+            plan.execute_peaks(dq, du, 640, 0, fq, fu, peak_index=idx, stream=torch.cuda.current_stream().cuda_stream)
+        g2.replay()
+        torch.cuda.synchronize()
+        check_cubes(fq.cpu().numpy(), fu.cpu().numpy(), FQ, FU, T, f"graph after a refused call {scheme}")
+        del g2
         plan.destroy()
 
 
