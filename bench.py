@@ -391,12 +391,15 @@ def main():
         h2d_bytes = 2 * hQ.numel() * 4
         d2h_bytes = 2 * hFQ.numel() * 4 + sum(v.numel() * 4 for v in hmaps.values())
         t_floor = max(h2d_bytes / (h2d * 1e9), d2h_bytes / (d2h * 1e9))
+        t_duplex = (h2d_bytes + d2h_bytes) / (duplex * 1e9)      # both directions busy at once share the link's duplex rate
         e2e = {"value": world * cfg.cmac / dt / 1e9, "unit": "GCMAC/s", "h2d_bytes_per_step": h2d_bytes,
                "d2h_bytes_per_step": d2h_bytes, "ms_per_step": dt * 1e3, "steps": k_e2e,
                "matches_device_path": ok, "api": "rmsynth_execute_host (pinned host buffers, 3 slots: H2D / kernels / D2H overlap)",
                "pcie": {"h2d_gbs": h2d, "d2h_gbs": d2h, "duplex_gbs": duplex,
                         "floor_ms": t_floor * 1e3, "frac_of_floor": t_floor / dt,
-                        "note": "pinned torch copies of 1 GiB measured in this run; floor = max(H2D bytes / H2D rate, D2H bytes / D2H rate)"}}
+                        "duplex_floor_ms": t_duplex * 1e3, "frac_of_duplex_floor": t_duplex / dt,
+                        "note": "pinned torch copies of 1 GiB measured in this run; floor = max(H2D bytes / H2D rate, D2H bytes / D2H rate); "
+                                "duplex_floor = (H2D + D2H bytes) / the rate with both directions running at once"}}
         del hQ, hU, hFQ, hFU, hmaps
         if not ok:
             print("bench.py: rmsynth_execute_host disagrees with the device-resident path", file=sys.stderr)
