@@ -203,7 +203,7 @@ rmsynth_status rmsynth_execute_fft(const rmsynth_plan *plan, const float *Q, con
  *   model_*, resid_*  DEVICE output cubes, same layout; rest_* likewise or both NULL
  *   n_iter            DEVICE [n_pix] iterations done per line of sight, or NULL
  * A line of sight holding a non-finite sample is passed through (model 0, residual = restored = input, 0
- * iterations).  Needs a uniform depth grid (else EUNSUPPORTED) of at most 14080 depths.  Only enqueues on
+ * iterations).  Needs a uniform depth grid (else EUNSUPPORTED) of at most 14336 depths.  Only enqueues on
  * `stream`, except the first call of a plan (and a change of fwhm), which builds the beam synchronously.
  * EINVAL: gain outside (0, 1], cutoff < 0, max_iter < 0, NULL cubes. */
 typedef struct {

@@ -10,7 +10,7 @@
 // Two kernels.  (a) n_phi <= 1024: one warp per line of sight, the residual in registers (lane l holds depths l + 32 i),
 // R, the Gaussian table and the eight warps' model arrays in shared memory, arg-max by warp shuffles; a CTA takes eight
 // consecutive pixels so that phi-major cubes are read and written in 32-byte sectors through a staging buffer.
-// (b) larger grids (the paper's 7000 depths): one CTA per line of sight, residual and model in shared memory.
+// (b) larger grids (the paper's 7000 depths): one CTA per line of sight, residual in registers, model in shared memory.
 #include <cmath>
 #include "common.cuh"
 
@@ -149,26 +149,51 @@ __global__ void __launch_bounds__(CL_WARPS * 32) rmclean_warp_kernel(const Clean
     }
 }
 
-// ---- (b) CTA per line of sight, residual and model in shared memory --------------------------------------------------
-constexpr int CB_THREADS = 256;
+// ---- (b) CTA per line of sight: residual in registers (thread t holds depths t + 512 i), model in shared memory -------
+// One pass over the residual per iteration: the subtraction of component j also finds the candidates for component
+// j + 1 (each thread keeps the largest |r|^2 of its own depths, strict > while its depths ascend = lowest index on
+// ties), so an iteration is NPT complex FMAs per thread, one block reduction and one __syncthreads (the per-warp
+// candidates are double-buffered by iteration parity).  The loop is latency-bound (one dependent beam load per FMA), so
+// the double-width beam sits in shared memory whenever it fits next to the model (n <= 9000: LDS instead of an L2 round
+// trip) and the CTA has 16 warps.  The restoring convolution visits only the non-zero model components of its window,
+// found through a bitmap of the model (one bit per depth), in ascending depth order (deterministic sums).
+constexpr int CB_THREADS = 512;
 
+template <int NPT, bool BEAM_SMEM>
 __global__ void __launch_bounds__(CB_THREADS) rmclean_block_kernel(const CleanArgs a) {
     extern __shared__ float2 smem2[];
     const int n = a.n_phi, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float2* r = smem2;            // [n] residual
-    float2* m = smem2 + n;        // [n] model
-    __shared__ float s_y[CB_THREADS / 32], s_q[CB_THREADS / 32], s_u[CB_THREADS / 32];
-    __shared__ int s_k[CB_THREADS / 32];
+    constexpr int NW = CB_THREADS / 32;
+    float2* m = smem2;                                            // [n] model
+    uint32_t* bits = reinterpret_cast<uint32_t*>(smem2 + n);      // [(n + 31) / 32 rounded up to even] bitmap of the model
+    const int n_words = (n + 31) >> 5;
+    float2* sR = smem2 + n + ((n_words + 1) >> 1);                // [2n - 1] beam (BEAM_SMEM)
+    __shared__ float s_y[2][NW], s_q[2][NW], s_u[2][NW];
+    __shared__ int s_k[2][NW];
     __shared__ float s_bad;
     const long long p = blockIdx.x;
     if (threadIdx.x == 0) s_bad = 0.f;
+    for (int i = threadIdx.x; i < n_words; i += CB_THREADS) bits[i] = 0u;
+    if (BEAM_SMEM)
+        for (int i = threadIdx.x; i < 2 * n - 1; i += CB_THREADS) sR[i] = __ldg(a.Rdw + i);
     __syncthreads();
+    float2 r[NPT];
     float bad = 0.f;
-    for (int k = threadIdx.x; k < n; k += CB_THREADS) {
-        const size_t o = cube_index(a, p, k);
-        const float2 v = make_float2(a.FQ[o], a.FU[o]);
-        r[k] = v; m[k] = make_float2(0.f, 0.f);
-        bad = fmaf(v.x, 0.f, fmaf(v.y, 0.f, bad));
+    float y = -1.f, cq = 0.f, cu = 0.f;     // this thread's candidate: largest |r|^2 of its depths
+    int kb = 0;
+#pragma unroll
+    for (int i = 0; i < NPT; ++i) {
+        const int k = threadIdx.x + i * CB_THREADS;
+        float2 v = make_float2(0.f, 0.f);
+        if (k < n) {
+            const size_t o = cube_index(a, p, k);
+            v = make_float2(a.FQ[o], a.FU[o]);
+            m[k] = make_float2(0.f, 0.f);
+            bad = fmaf(v.x, 0.f, fmaf(v.y, 0.f, bad));
+            const float t = fmaf(v.x, v.x, v.y * v.y);
+            if (t > y) { y = t; kb = k; cq = v.x; cu = v.y; }
+        }
+        r[i] = v;
     }
     if (!(bad == 0.f)) s_bad = 1.f;
     __syncthreads();
@@ -176,13 +201,7 @@ __global__ void __launch_bounds__(CB_THREADS) rmclean_block_kernel(const CleanAr
     const int c0 = n - 1;
     int it = 0;
     while (finite && it < a.max_iter) {
-        float y = -1.f, cq = 0.f, cu = 0.f;
-        int kb = 0;
-        for (int k = threadIdx.x; k < n; k += CB_THREADS) {
-            const float2 v = r[k];
-            const float t = fmaf(v.x, v.x, v.y * v.y);
-            if (t > y) { y = t; kb = k; cq = v.x; cu = v.y; }
-        }
+        const int par = it & 1;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             const float oy = __shfl_xor_sync(0xffffffffu, y, o), oq = __shfl_xor_sync(0xffffffffu, cq, o),
@@ -190,39 +209,57 @@ __global__ void __launch_bounds__(CB_THREADS) rmclean_block_kernel(const CleanAr
             const int ok = __shfl_xor_sync(0xffffffffu, kb, o);
             if (oy > y || (oy == y && ok < kb)) { y = oy; kb = ok; cq = oq; cu = ou; }
         }
-        if (lane == 0) { s_y[warp] = y; s_k[warp] = kb; s_q[warp] = cq; s_u[warp] = cu; }
+        if (lane == 0) { s_y[par][warp] = y; s_k[par][warp] = kb; s_q[par][warp] = cq; s_u[par][warp] = cu; }
         __syncthreads();
-        y = s_y[0]; kb = s_k[0]; cq = s_q[0]; cu = s_u[0];
+        y = s_y[par][0]; kb = s_k[par][0]; cq = s_q[par][0]; cu = s_u[par][0];
 #pragma unroll
-        for (int w2 = 1; w2 < CB_THREADS / 32; ++w2)
-            if (s_y[w2] > y || (s_y[w2] == y && s_k[w2] < kb)) { y = s_y[w2]; kb = s_k[w2]; cq = s_q[w2]; cu = s_u[w2]; }
-        __syncthreads();                                  // everybody has read the candidates
-        if (y < a.cutoff2) break;
+        for (int w2 = 1; w2 < NW; ++w2)
+            if (s_y[par][w2] > y || (s_y[par][w2] == y && s_k[par][w2] < kb)) { y = s_y[par][w2]; kb = s_k[par][w2]; cq = s_q[par][w2]; cu = s_u[par][w2]; }
+        if (y < a.cutoff2) break;                              // C3: stop before subtracting
         cq *= a.gain; cu *= a.gain;
-        if (threadIdx.x == 0) { float2 v = m[kb]; v.x += cq; v.y += cu; m[kb] = v; }
-        const float2* beam = a.Rdw + (c0 - kb);
-        for (int k = threadIdx.x; k < n; k += CB_THREADS) {
-            const float2 b = __ldg(beam + k);
-            float2 v = r[k];
-            v.x -= cq * b.x - cu * b.y;
-            v.y -= cq * b.y + cu * b.x;
-            r[k] = v;
+        if (threadIdx.x == 0) { float2 v = m[kb]; v.x += cq; v.y += cu; m[kb] = v; bits[kb >> 5] |= 1u << (kb & 31); }
+        const float2* beam = (BEAM_SMEM ? sR : a.Rdw) + (c0 - kb);
+        const float gq = cq, gu = cu;
+        y = -1.f; kb = 0; cq = 0.f; cu = 0.f;
+#pragma unroll
+        for (int i = 0; i < NPT; ++i) {
+            const int k = threadIdx.x + i * CB_THREADS;
+            if (k < n) {
+                const float2 b = BEAM_SMEM ? beam[k] : __ldg(beam + k);
+                float2 v = r[i];
+                v.x -= gq * b.x - gu * b.y;
+                v.y -= gq * b.y + gu * b.x;
+                r[i] = v;
+                const float t = fmaf(v.x, v.x, v.y * v.y);
+                if (t > y) { y = t; kb = k; cq = v.x; cu = v.y; }
+            }
         }
-        __syncthreads();
         ++it;
     }
-    __syncthreads();
+    __syncthreads();                                           // the model and its bitmap are complete
     if (a.n_iter && threadIdx.x == 0) a.n_iter[p] = it;
-    for (int k = threadIdx.x; k < n; k += CB_THREADS) {
+#pragma unroll
+    for (int i = 0; i < NPT; ++i) {
+        const int k = threadIdx.x + i * CB_THREADS;
+        if (k >= n) continue;
         const size_t o = cube_index(a, p, k);
-        const float2 rv = r[k], mv = m[k];
+        const float2 rv = r[i], mv = m[k];
         a.mq[o] = mv.x; a.mu[o] = mv.y; a.rq[o] = rv.x; a.ru[o] = rv.y;
         if (a.sq) {
             float sq = rv.x, su = rv.y;
             const int lo = max(0, k - a.gauss_reach), hi = min(n - 1, k + a.gauss_reach);
-            for (int j = lo; j <= hi; ++j) {
-                const float2 c = m[j];
-                if (c.x != 0.f || c.y != 0.f) { const float g = __ldg(a.gauss + (j > k ? j - k : k - j)); sq = fmaf(c.x, g, sq); su = fmaf(c.y, g, su); }
+            for (int wd = lo >> 5; wd <= hi >> 5; ++wd) {
+                uint32_t bb = bits[wd];
+                if (wd == lo >> 5) bb &= 0xFFFFFFFFu << (lo & 31);
+                if (wd == hi >> 5) bb &= 0xFFFFFFFFu >> (31 - (hi & 31));
+                while (bb) {                                     // ascending depth order
+                    const int j = wd * 32 + __ffs(bb) - 1;
+                    bb &= bb - 1;
+                    const float2 c = m[j];
+                    const float g = __ldg(a.gauss + (j > k ? j - k : k - j));
+                    sq = fmaf(c.x, g, sq);
+                    su = fmaf(c.y, g, su);
+                }
             }
             a.sq[o] = sq; a.su[o] = su;
         }
@@ -323,11 +360,23 @@ extern "C" rmsynth_status rmsynth_rmclean(const rmsynth_plan* plan, const float*
 #undef CL_GO
         RMS_LAUNCH_CHECK("rmclean_warp_kernel");
     } else {
-        const size_t smem = sizeof(float2) * 2 * (size_t)n;
-        if (smem > 220 * 1024) return fail(RMSYNTH_EUNSUPPORTED, "RM-CLEAN: more than 14080 depths do not fit in shared memory");
+        const int n_words = (n + 31) >> 5;
+        const size_t smem_small = sizeof(float2) * ((size_t)n + ((n_words + 1) >> 1));
+        const size_t smem_beam = smem_small + sizeof(float2) * (size_t)(2 * n - 1);
+        const bool beam_smem = smem_beam <= 220 * 1024;
+        const size_t smem = beam_smem ? smem_beam : smem_small;
+        if (n > 28 * CB_THREADS) return fail(RMSYNTH_EUNSUPPORTED, "RM-CLEAN: more than 14336 depths do not fit in the registers of a CTA");
         if (n_pix > 0x7fffffffLL) return fail(RMSYNTH_EINVAL, "n_pix too large");
-        RMS_CUDA(cudaFuncSetAttribute(rmclean_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        rmclean_block_kernel<<<(unsigned)n_pix, CB_THREADS, smem, st>>>(a);
+#define CB_GO(NPT, BS)                                                                                                            \
+        do {                                                                                                                      \
+            RMS_CUDA(cudaFuncSetAttribute(rmclean_block_kernel<NPT, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            rmclean_block_kernel<NPT, BS><<<(unsigned)n_pix, CB_THREADS, smem, st>>>(a);                                          \
+        } while (0)
+        if (n <= 4 * CB_THREADS) CB_GO(4, true);
+        else if (n <= 8 * CB_THREADS) CB_GO(8, true);
+        else if (n <= 16 * CB_THREADS) { if (beam_smem) CB_GO(16, true); else CB_GO(16, false); }
+        else CB_GO(28, false);
+#undef CB_GO
         RMS_LAUNCH_CHECK("rmclean_block_kernel");
     }
     return RMSYNTH_OK;
