@@ -121,7 +121,7 @@ def workload_dict(cid, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config, 1-based (default 5 = configs[4], the target cube)")
     ap.add_argument("--scheme", default="auto", choices=["auto", "f16x3", "tf32x3", "fp32_table", "fp32_sincos"])
