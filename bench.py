@@ -42,16 +42,34 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def ncu_evidence(config: int, scheme: str, source_hash: str):
+TENSOR_PATH_FILES = ("tc_gemm.cu", "tc_gemm2.cu", "tc_gemm3.cu", "tc_common.cuh", "tc_epilogue.cuh", "peak_refine.cuh", "peaks.cu",
+                     "common.cuh", "execute.cu", "plan.cu")
+
+
+def tensor_path_hash() -> str:
+    """SHA-256 (16 hex digits) of the sources the execute path is compiled from (the tensor kernels, their epilogue, the
+    peak kernels, dispatch and plan) -- what an ncu capture of that path depends on.  Edits to rmclean.cu or fft_variant.cu
+    do not change it."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1810_06250_b200", "csrc")
+    for name in TENSOR_PATH_FILES:
+        h.update(name.encode())
+        with open(os.path.join(csrc, name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_evidence(config: int, scheme: str):
     """dram bytes / tensor-pipe activity of the dominant kernel from the committed ncu capture -- only if that capture
-    was taken with the library built from the sources this run uses (content hash); else None: stale evidence is no evidence."""
+    was taken with the tensor-path sources this run uses (content hash); else None: stale evidence is no evidence."""
     try:
         with open(NCU_FILE) as f:
             d = json.load(f)
     except OSError:
         return None
     e = d.get("captures", {}).get(f"{config}:{scheme}")
-    if not e or e.get("source_hash") != source_hash:
+    if not e or e.get("tensor_path_hash") != tensor_path_hash():
         return None
     return e
 
@@ -452,7 +470,7 @@ def main():
     peaks, peaks_src = load_peaks()
     kern_ms = float(np.mean(per_step))
     src_hash = libbuild.source_hash()
-    ev = ncu_evidence(a.config, a.scheme, src_hash)
+    ev = ncu_evidence(a.config, a.scheme)
     if scheme in (b.SCHEME_TF32X3, b.SCHEME_F16X3):
         achieved = TENSOR_FLOP_PER_CMAC * cfg.cmac / (kern_ms * 1e-3) / 1e12
         f16 = scheme == b.SCHEME_F16X3
@@ -473,7 +491,7 @@ def main():
                         f"timed region is {a.steps} back-to-back {kern_ms:.1f} ms kernels under the 1 kW power cap (see clocks), where the same "
                         f"file's SUSTAINED figure {peaks.get('bf16_tflops_sustained', 0):.0f} TF applies: frac_of_sustained_peak; traffic and "
                         f"tensor_pipe_active_pct_ncu come from profiles/r02_ncu_summary.json and are null unless that capture was taken "
-                        f"with the library built from these very sources (content hash {src_hash})"}
+                        f"with these very tensor-path sources (content hash {tensor_path_hash()}; library {src_hash})"}
     else:
         achieved = FP32_FLOP_PER_CMAC * cfg.cmac / (kern_ms * 1e-3) / 1e12
         peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12

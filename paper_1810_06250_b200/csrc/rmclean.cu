@@ -211,10 +211,18 @@ __global__ void __launch_bounds__(CB_THREADS) rmclean_block_kernel(const CleanAr
         }
         if (lane == 0) { s_y[par][warp] = y; s_k[par][warp] = kb; s_q[par][warp] = cq; s_u[par][warp] = cu; }
         __syncthreads();
-        y = s_y[par][0]; kb = s_k[par][0]; cq = s_q[par][0]; cu = s_u[par][0];
+        {   // every warp merges the NW = 16 candidates with shuffles (lane l < 16 takes warp l's): 4 steps instead of 16 reads
+            const int wsrc = lane & (NW - 1);
+            y = s_y[par][wsrc]; kb = s_k[par][wsrc];
+            int wb = wsrc;
 #pragma unroll
-        for (int w2 = 1; w2 < NW; ++w2)
-            if (s_y[par][w2] > y || (s_y[par][w2] == y && s_k[par][w2] < kb)) { y = s_y[par][w2]; kb = s_k[par][w2]; cq = s_q[par][w2]; cu = s_u[par][w2]; }
+            for (int o = NW / 2; o > 0; o >>= 1) {
+                const float oy = __shfl_xor_sync(0xffffffffu, y, o);
+                const int ok = __shfl_xor_sync(0xffffffffu, kb, o), ow = __shfl_xor_sync(0xffffffffu, wb, o);
+                if (oy > y || (oy == y && ok < kb)) { y = oy; kb = ok; wb = ow; }
+            }
+            cq = s_q[par][wb]; cu = s_u[par][wb];
+        }
         if (y < a.cutoff2) break;                              // C3: stop before subtracting
         cq *= a.gain; cu *= a.gain;
         if (threadIdx.x == 0) { float2 v = m[kb]; v.x += cq; v.y += cu; m[kb] = v; bits[kb >> 5] |= 1u << (kb & 31); }
