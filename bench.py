@@ -264,7 +264,10 @@ def main():
 
     # ------------------------------------------------------------------ the headline workload
     Q, U, FQ, FU, maps = alloc(cfg)
+    t_plan = time.perf_counter()
     plan = b.Plan(nu, w, phi, scheme=scheme_id[a.scheme])
+    torch.cuda.synchronize()
+    plan_create_ms = (time.perf_counter() - t_plan) * 1e3     # lambda^2, K, lambda_0^2, phase matrix, operand blobs, R(phi): once per grid
     scheme = plan.scheme                      # what "auto" resolved to
     a.scheme = scheme_name[scheme]
     per_step, total_ms, launches, t_begin, t_end = timed(plan, cfg, Q, U, FQ, FU, maps, a.steps, a.warmup)
@@ -513,7 +516,7 @@ def main():
            "config": dict(workload, scheme=a.scheme, l2="inputs and outputs larger than L2 (no flush needed)"
                           if 8 * cfg.n_pix * (cfg.n_chan + cfg.n_phi) > 126e6 else "fits in L2", peaks=peaks_on,
                           outputs="FQ + FU cubes" + (" + peak |F| / peak phi / PA maps (fused)" if peaks_on else "")),
-           "mpix_per_s": world * cfg.n_pix / (ms_step * 1e-3) / 1e6,
+           "mpix_per_s": world * cfg.n_pix / (ms_step * 1e-3) / 1e6, "plan_create_ms": plan_create_ms,
            "roofline": roof, "alt_scheme": alt, "secondary": secondary, "extras": extras, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
            "clocks": clocks, "library": b.rmsynth_version(),
            "paper_context": "P100 compute-only 10.6-116 GCMAC/s (Table 1, P:L302-304), other hardware: context only"}
