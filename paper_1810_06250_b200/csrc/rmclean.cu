@@ -36,7 +36,7 @@ __device__ __forceinline__ size_t cube_index(const CleanArgs& a, long long p, in
 constexpr int CL_WARPS = 8;
 
 template <int NPL>
-__global__ void __launch_bounds__(CL_WARPS * 32) rmclean_warp_kernel(const CleanArgs a) {
+__global__ void __launch_bounds__(CL_WARPS * 32, NPL <= 16 ? 3 : 1) rmclean_warp_kernel(const CleanArgs a) {
     extern __shared__ float2 smem2[];
     const int n = a.n_phi, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float2* sR = smem2;                                   // [2n - 1]
@@ -81,12 +81,13 @@ __global__ void __launch_bounds__(CL_WARPS * 32) rmclean_warp_kernel(const Clean
             const float v = lane + 32 * i < n ? fmaf(rq[i], rq[i], ru[i] * ru[i]) : -1.f;
             if (v > y) { y = v; kb = lane + 32 * i; cq = rq[i]; cu = ru[i]; }
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const float oy = __shfl_xor_sync(0xffffffffu, y, o), oq = __shfl_xor_sync(0xffffffffu, cq, o),
-                        ou = __shfl_xor_sync(0xffffffffu, cu, o);
-            const int ok = __shfl_xor_sync(0xffffffffu, kb, o);
-            if (oy > y || (oy == y && ok < kb)) { y = oy; kb = ok; cq = oq; cu = ou; }
+        {   // two warp reductions (redux.sync) instead of five shuffle stages: |r|^2 >= 0, so its bit pattern orders like an
+            // unsigned integer; among the lanes holding the maximum the lowest depth wins; its owner is lane kb & 31
+            const unsigned yb = __float_as_uint(y), ymax = __reduce_max_sync(0xffffffffu, yb);
+            kb = (int)__reduce_min_sync(0xffffffffu, yb == ymax ? (unsigned)kb : 0x7fffffffu);
+            y = __uint_as_float(ymax);
+            cq = __shfl_sync(0xffffffffu, cq, kb & 31);
+            cu = __shfl_sync(0xffffffffu, cu, kb & 31);
         }
         if (y < a.cutoff2) break;
         cq *= a.gain; cu *= a.gain;                       // C4
