@@ -203,25 +203,18 @@ __global__ void __launch_bounds__(CB_THREADS) rmclean_block_kernel(const CleanAr
     int it = 0;
     while (finite && it < a.max_iter) {
         const int par = it & 1;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const float oy = __shfl_xor_sync(0xffffffffu, y, o), oq = __shfl_xor_sync(0xffffffffu, cq, o),
-                        ou = __shfl_xor_sync(0xffffffffu, cu, o);
-            const int ok = __shfl_xor_sync(0xffffffffu, kb, o);
-            if (oy > y || (oy == y && ok < kb)) { y = oy; kb = ok; cq = oq; cu = ou; }
+        {   // warp level: two redux.sync reductions (|r|^2 >= 0 orders like its bit pattern; lowest depth among the maxima)
+            const unsigned yb = __float_as_uint(y), ymax = __reduce_max_sync(0xffffffffu, yb);
+            const unsigned kmin = __reduce_min_sync(0xffffffffu, yb == ymax ? (unsigned)kb : 0x7fffffffu);
+            if (yb == ymax && (unsigned)kb == kmin) { s_y[par][warp] = y; s_k[par][warp] = kb; s_q[par][warp] = cq; s_u[par][warp] = cu; }
         }
-        if (lane == 0) { s_y[par][warp] = y; s_k[par][warp] = kb; s_q[par][warp] = cq; s_u[par][warp] = cu; }
         __syncthreads();
-        {   // every warp merges the NW = 16 candidates with shuffles (lane l < 16 takes warp l's): 4 steps instead of 16 reads
+        {   // every warp merges the NW = 16 candidates the same way (lane l takes warp l & 15's)
             const int wsrc = lane & (NW - 1);
-            y = s_y[par][wsrc]; kb = s_k[par][wsrc];
-            int wb = wsrc;
-#pragma unroll
-            for (int o = NW / 2; o > 0; o >>= 1) {
-                const float oy = __shfl_xor_sync(0xffffffffu, y, o);
-                const int ok = __shfl_xor_sync(0xffffffffu, kb, o), ow = __shfl_xor_sync(0xffffffffu, wb, o);
-                if (oy > y || (oy == y && ok < kb)) { y = oy; kb = ok; wb = ow; }
-            }
+            const unsigned yb = __float_as_uint(s_y[par][wsrc]), ymax = __reduce_max_sync(0xffffffffu, yb);
+            const unsigned kc = (unsigned)s_k[par][wsrc], kmin = __reduce_min_sync(0xffffffffu, yb == ymax ? kc : 0x7fffffffu);
+            const int wb = __ffs(__ballot_sync(0xffffffffu, yb == ymax && kc == kmin)) - 1;
+            y = __uint_as_float(ymax); kb = (int)kmin;
             cq = s_q[par][wb]; cu = s_u[par][wb];
         }
         if (y < a.cutoff2) break;                              // C3: stop before subtracting
