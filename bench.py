@@ -419,8 +419,10 @@ def main():
                "pcie": {"h2d_gbs": h2d, "d2h_gbs": d2h, "duplex_gbs": duplex,
                         "floor_ms": t_floor * 1e3, "frac_of_floor": t_floor / dt,
                         "duplex_floor_ms": t_duplex * 1e3, "frac_of_duplex_floor": t_duplex / dt,
+                        "frac_of_tighter_floor": max(t_floor, t_duplex) / dt,
                         "note": "pinned torch copies of 1 GiB measured in this run; floor = max(H2D bytes / H2D rate, D2H bytes / D2H rate); "
-                                "duplex_floor = (H2D + D2H bytes) / the rate with both directions running at once"}}
+                                "duplex_floor = (H2D + D2H bytes) / the rate with both directions running at once (binds when the two directions carry similar bytes); "
+                                "the tighter of the two is the bound"}}
         del hQ, hU, hFQ, hFU, hmaps
         if not ok:
             print("bench.py: rmsynth_execute_host disagrees with the device-resident path", file=sys.stderr)
