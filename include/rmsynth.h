@@ -218,6 +218,35 @@ rmsynth_status rmsynth_rmclean(const rmsynth_plan *plan, const float *FQ, const 
                                float *model_u, float *resid_q, float *resid_u, float *rest_q,
                                float *rest_u, int *n_iter, void *stream);
 
+/* Peak maps (Eq. 14, Eq. 17; same rules as rmsynth_execute_peaks) of FQ/FU cubes that are
+ * already in device memory -- what rmsynth_execute, rmsynth_execute_fft or rmsynth_rmclean wrote -- through a call
+ * that ALLOCATES NOTHING, now or later.  It exists for callers that cannot call cudaMalloc once they are running: a
+ * framework whose own pool took the whole device at start-up (a library's late cudaMalloc just fails there), a
+ * client under a fixed device-memory cap (MPS / MIG share), a real-time loop that cannot take cudaMalloc's
+ * device-wide synchronisation and millisecond latency.  Every other call that produces maps fetches its workspace
+ * with cudaMalloc the first time it sees a (stream, size); this one keeps its per-(pixel, depth segment) records in
+ * a 32 MiB array inside the library image.
+ *   plan        supplies the depth grid, n_phi and lambda_0^2 (allocated when the plan was created, not here)
+ *   FQ, FU      DEVICE cubes, laid out per the RMSYNTH_OUT_* bit of `layout` (the RMSYNTH_IN_* bit is ignored)
+ *   ld          row pitch in floats: F[k*ld + p] (OUT_PHI_MAJOR, ld >= n_pix) or F[p*ld + k] (OUT_LOS_MAJOR,
+ *               ld >= n_phi); 0 = dense.  With a pointer offset it selects a slab of pixels of a larger cube.
+ *   peak_*, pa_*  DEVICE [n_pix], any may be NULL, at least one must not be
+ * LIMIT: n_pix <= 1 048 576 per call (the records must fit the array); more is EINVAL with a message that says so --
+ * split the image into slabs.  Cost: 32 MiB of every GPU on which the library is loaded, held until the process
+ * exits, used or not.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, which also makes the driver load
+ * the module that holds the array).  Make that call during start-up, before any stream capture begins; later calls
+ * only enqueue two kernels on `stream`.  Never synchronises, never calls cudaMalloc / cudaFree.
+ * The array is shared by ALL calls on a device, whatever the plan or stream, and is left holding the last call's
+ * records.  A call depends on none of that (it overwrites every record it reads), but two calls that may run on the
+ * GPU at the same time -- different streams, or different host threads without ordering between them -- race on it
+ * and return garbage: keep calls to this entry point on one stream, or order them with events.
+ * n_pix == 0 is a successful no-op.  EINVAL: NULL plan or cubes, n_pix < 0 or beyond the limit, unknown layout bits,
+ * ld below the dense length, no map requested. */
+rmsynth_status rmsynth_peaks_static(const rmsynth_plan *plan, const float *FQ, const float *FU, long long n_pix,
+                                    long long ld, int layout, float *peak_amp, float *peak_phi,
+                                    float *pa_lambda0, float *pa_zero, int *peak_index, void *stream);
+
 /* R(phi) of Eq. 12 in FP64.  phi_eval HOST [n] or NULL for the plan grid (then n must be
  * n_phi); R_re, R_im HOST [n].  Synchronous. */
 rmsynth_status rmsynth_rmsf(const rmsynth_plan *plan, const double *phi_eval, int n,

@@ -27,7 +27,7 @@ SCHEME_AUTO, SCHEME_TF32X3, SCHEME_F16X3, SCHEME_FP32_TABLE, SCHEME_FP32_SINCOS 
 
 EXPORTS = ["rmsynth_plan_create", "rmsynth_plan_destroy", "rmsynth_plan_info", "rmsynth_plan_phase_matrix",
            "rmsynth_execute", "rmsynth_execute_peaks", "rmsynth_execute_ex", "rmsynth_execute_host", "rmsynth_execute_stream",
-           "rmsynth_rmsf", "rmsynth_rmclean", "rmsynth_execute_fft",
+           "rmsynth_rmsf", "rmsynth_rmclean", "rmsynth_execute_fft", "rmsynth_peaks_static",
            "rmsynth_launch_count", "rmsynth_strerror", "rmsynth_last_error", "rmsynth_version"]
 
 
@@ -67,6 +67,7 @@ class FftParams(C.Structure):
 
 _lib.rmsynth_execute_fft.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, _fp, _fp, C.POINTER(FftParams), _vp]
 _lib.rmsynth_rmclean.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_int, C.POINTER(CleanParams), _fp, _fp, _fp, _fp, _fp, _fp, _ip, _vp]
+_lib.rmsynth_peaks_static.argtypes = [_vp, _fp, _fp, C.c_longlong, C.c_longlong, C.c_int, _fp, _fp, _fp, _fp, _ip, _vp]
 _lib.rmsynth_rmsf.argtypes = [_vp, _dp, C.c_int, _dp, _dp]
 _lib.rmsynth_launch_count.argtypes = [C.c_int]
 _lib.rmsynth_launch_count.restype = C.c_longlong
@@ -186,6 +187,13 @@ class Plan:
         prm = CleanParams(C.sizeof(CleanParams), gain, cutoff, max_iter, fwhm)
         _check(_lib.rmsynth_rmclean(self._h, _ptr(FQ), _ptr(FU), n_pix, layout, C.byref(prm), _ptr(model_q), _ptr(model_u),
                                     _ptr(resid_q), _ptr(resid_u), _ptr(rest_q), _ptr(rest_u), _ptr(n_iter), stream))
+
+    def peaks_static(self, FQ, FU, n_pix, layout, ld=0, peak_amp=None, peak_phi=None, pa_lambda0=None, pa_zero=None,
+                     peak_index=None, stream=None):
+        """Peak maps of DEVICE cubes through the entry point that never allocates (records in the library's static
+        32 MiB array; n_pix <= 1048576 per call; calls that may overlap on the GPU race on that array)."""
+        _check(_lib.rmsynth_peaks_static(self._h, _ptr(FQ), _ptr(FU), n_pix, ld, layout, _ptr(peak_amp), _ptr(peak_phi),
+                                         _ptr(pa_lambda0), _ptr(pa_zero), _ptr(peak_index), stream))
 
     def execute_stream(self, layout, outputs, fill, drain):
         """fill(i, Q, U, max_pix) -> n and drain(i, n, out) are Python callables; Q, U are numpy views of the
