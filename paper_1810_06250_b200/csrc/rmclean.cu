@@ -83,8 +83,11 @@ __global__ void __launch_bounds__(CL_WARPS * 32, NPL <= 16 ? 3 : 1) rmclean_warp
         }
         {   // two warp reductions (redux.sync) instead of five shuffle stages: |r|^2 >= 0, so its bit pattern orders like an
             // unsigned integer; among the lanes holding the maximum the lowest depth wins; its owner is lane kb & 31
-            const unsigned yb = __float_as_uint(y), ymax = __reduce_max_sync(0xffffffffu, yb);
-            kb = (int)__reduce_min_sync(0xffffffffu, yb == ymax ? (unsigned)kb : 0x7fffffffu);
+            // a lane beyond the grid (n_phi < 32) holds no depth: its -1 sentinel would sort above every real value as an
+            // unsigned integer, so it enters the reductions as the lowest value and never as a candidate depth
+            const bool has = y >= 0.f;
+            const unsigned yb = has ? __float_as_uint(y) : 0u, ymax = __reduce_max_sync(0xffffffffu, yb);
+            kb = (int)__reduce_min_sync(0xffffffffu, has && yb == ymax ? (unsigned)kb : 0x7fffffffu);
             y = __uint_as_float(ymax);
             cq = __shfl_sync(0xffffffffu, cq, kb & 31);
             cu = __shfl_sync(0xffffffffu, cu, kb & 31);

@@ -66,7 +66,7 @@ def check(oracle_mod, op, FQ, FU, got, ref, gain, cutoff, max_iter, what):
     # properties, every line of sight
     # model * R: the beam centred on depth j is R((k - j) dphi) (reading C1) -- one RMSF call on the double-width grid, then
     # a sum over the (few) non-zero components of every line of sight
-    dphi = float(op.phi[1] - op.phi[0])
+    dphi = float(op.phi[1] - op.phi[0]) if n > 1 else 1.0
     Rdw = oracle_mod.rmsf(op, dphi * (np.arange(2 * n - 1) - (n - 1)))
     back = got["residual"].copy()
     for p_, j_ in zip(*np.nonzero(got["model"])):
@@ -109,6 +109,34 @@ def test_rmclean_matches_oracle(b, oracle_mod, lout, cfg_id, n_pix, n_phi, gain,
     got = run_clean(b, plan, FQ, FU, lout, gain, cutoff, max_iter, fwhm)
     frac = check(oracle_mod, op, FQ, FU, got, ref, gain, cutoff, max_iter, f"cfg{cfg_id} {phi.size} depths {lout}")
     print(f"cfg{cfg_id} {phi.size} depths {lout}: {frac:.2f} of the lines of sight decision-stable, iterations {ref['n_iter'].min()}..{ref['n_iter'].max()}")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("lout", ["los", "phi"])
+@pytest.mark.parametrize("n_phi", [1, 2, 5, 31, 32, 33])
+def test_rmclean_grids_narrower_than_a_warp(b, oracle_mod, lout, n_phi):
+    """Fewer depths than lanes: the lanes without a depth must never win the arg-max (their sentinel once sorted above
+    every real |r|^2 in the unsigned reduction and ended the loop before its first iteration).  1, 2, 5 and 31 depths,
+    with 32 and 33 as the neighbours on the other side; band and spacing chosen so that the RMSF is a few samples
+    wide.  Noise spectra plus one source, seeded here and handed to both sides."""
+    nu = np.linspace(1.0e9, 1.8e9, 96)
+    dphi = 25.0
+    phi = (np.arange(n_phi) - n_phi // 2) * dphi
+    op = oracle_mod.make_plan(nu, None, phi)
+    rng = np.random.default_rng(100 + n_phi)
+    n_pix = 37
+    lam2 = (299792458.0 / nu) ** 2
+    src = rng.uniform(phi[0], phi[-1] + 1e-9, n_pix)[:, None]
+    P = np.exp(2j * src * lam2[None, :]) * rng.uniform(0.5, 2.0, (n_pix, 1)) + 0.3 * (rng.standard_normal((n_pix, 96)) + 1j * rng.standard_normal((n_pix, 96)))
+    FQ, FU = oracle_mod.synth_table(op, np.ascontiguousarray(P.real, dtype=np.float32), np.ascontiguousarray(P.imag, dtype=np.float32))
+    FQ, FU = FQ.astype(np.float32), FU.astype(np.float32)
+    gain, max_iter, fwhm = 0.2, 30, 2.5 * dphi
+    cutoff = 0.25 * float(np.median(np.abs(FQ.astype(np.float64) + 1j * FU).max(axis=1)))
+    ref = oracle_mod.rmclean(op, FQ, FU, gain=gain, cutoff=cutoff, max_iter=max_iter, fwhm=fwhm)
+    assert ref["n_iter"].max() > 0, "the case must iterate to test anything"
+    plan = b.Plan(nu, None, phi, scheme=b.SCHEME_FP32_TABLE)
+    got = run_clean(b, plan, FQ, FU, lout, gain, cutoff, max_iter, fwhm)
+    check(oracle_mod, op, FQ, FU, got, ref, gain, cutoff, max_iter, f"{n_phi} depths {lout}")
     plan.destroy()
 
 
