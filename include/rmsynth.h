@@ -56,7 +56,14 @@ enum {
     RMSYNTH_SCHEME_TF32X3 = 1,      /* tcgen05 tensor cores, split-precision 3xTF32,     */
                                     /* FP32 accumulate in TMEM                           */
     RMSYNTH_SCHEME_F16X3 = 2,       /* tcgen05 tensor cores, block-scaled FP16 hi/lo split    */
-                                    /* (3 products at twice the TF32 rate), FP32 accumulate   */
+                                    /* (3 products at twice the TF32 rate), FP32 accumulate.  */
+                                    /* Each 32-channel chunk of a line of sight is scaled by  */
+                                    /* its own maximum, floored at 2^(eB - 112) ~ 1e-27 (eB = */
+                                    /* the plan's power-of-two scale of K w, 23-24 for a few  */
+                                    /* hundred channels): a smaller chunk is scaled by the    */
+                                    /* floor's power and loses one bit per factor two under   */
+                                    /* it (parity-grade to ~1e-28, plain FP16 accuracy below, */
+                                    /* never flushed to zero); the other schemes have no floor */
     RMSYNTH_SCHEME_FP32_TABLE = 3,  /* CUDA cores, FP32 FMA, reads the plan's cos/sin    */
     RMSYNTH_SCHEME_FP32_SINCOS = 4  /* CUDA cores, sincos on the fly, one (pixel,phi)    */
                                     /* per thread -- the paper's kernel shape    */

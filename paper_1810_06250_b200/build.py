@@ -8,7 +8,7 @@ is compiled into the library (rmsynth_version() reports it) and written next to 
 whenever the hash of the sources on disk differs from the one the binary was built from.
 
 --timeline builds librmsynth_timeline.so, the same sources with -DRMSYNTH_TIMELINE (per-role clock64
-stamps in the FP16 tensor kernel, read by paper_1810_06250_b200/timeline.py).  Debug only.
+stamps in the FP16 tensor kernel, read back through rmsynth_timeline_read).  Debug only.
 """
 from __future__ import annotations
 

@@ -69,18 +69,26 @@ struct HostPipe {
     size_t in_bytes = 0, out_bytes = 0;
 };
 
+// Streams and events of the host pipeline, created on first use.  The HostPipe is attached to the plan only once every
+// create has succeeded: a failure half-way releases what exists and leaves the plan without one, so the next call starts
+// over instead of running with null streams (the legacy default stream) and null events.
 static rmsynth_status pipe_get(const rmsynth_plan* p, HostPipe** out) {
     if (!p->host_pipe) {
         HostPipe* hp = new HostPipe;
-        p->host_pipe = hp;
-        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_in, cudaStreamNonBlocking));
-        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_run, cudaStreamNonBlocking));
-        RMS_CUDA(cudaStreamCreateWithFlags(&hp->s_out, cudaStreamNonBlocking));
-        for (int b = 0; b < kSlots; ++b) {
-            RMS_CUDA(cudaEventCreateWithFlags(&hp->in_done[b], cudaEventDisableTiming));
-            RMS_CUDA(cudaEventCreateWithFlags(&hp->run_done[b], cudaEventDisableTiming));
-            RMS_CUDA(cudaEventCreateWithFlags(&hp->out_done[b], cudaEventDisableTiming));
+        cudaError_t e = cudaStreamCreateWithFlags(&hp->s_in, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&hp->s_run, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&hp->s_out, cudaStreamNonBlocking);
+        for (int b = 0; b < kSlots && e == cudaSuccess; ++b) {
+            e = cudaEventCreateWithFlags(&hp->in_done[b], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->run_done[b], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->out_done[b], cudaEventDisableTiming);
         }
+        if (e != cudaSuccess) {
+            p->host_pipe = hp;                                // host_pipe_free releases whatever was created and detaches it
+            host_pipe_free(const_cast<rmsynth_plan*>(p));
+            RMS_CUDA(e);
+        }
+        p->host_pipe = hp;
     }
     *out = static_cast<HostPipe*>(p->host_pipe);
     return RMSYNTH_OK;

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda.h>
 #include <cstdint>
+#include <cstdlib>
 #include <cuda_runtime.h>
 
 namespace rms {
@@ -95,6 +96,14 @@ __device__ __forceinline__ float rn_tf32(float x) {   // round-to-nearest(-even)
     return __uint_as_float(u & 0xFFFFE000u);
 }
 
+
+// Experiment knobs exist only in a -DRMSYNTH_EXPERIMENT build, which build() never makes: the product library reads no
+// environment variable, so a call, a later call and a captured graph always take the same path.
+#ifdef RMSYNTH_EXPERIMENT
+static inline const char* experiment_env(const char* name) { return getenv(name); }
+#else
+static inline const char* experiment_env(const char*) { return nullptr; }
+#endif
 
 // Static "gang" schedule of the (pixel-tile pair, depth tile) work items over the CTA pairs of the grid.
 // T = depth tiles per pixel-tile pair, G = gang size (a divisor of T).  The first S = floor(n_clusters / G) G clusters

@@ -160,8 +160,8 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
         RMS_CUDA(cudaMemsetAsync(tile_sync, 0, sizeof(int) * (size_t)n_pairs, st));
     }
     const int T = f16 ? p->tc3.n_phi_tiles : p->tc.n_phi_tiles;
-    const char* lag_env = getenv("RMSYNTH_SYNC_LAG");        // EXPERIMENT knobs
-    const char* gang_env = getenv("RMSYNTH_GANG");
+    const char* lag_env = experiment_env("RMSYNTH_SYNC_LAG");   // compiled out of the product build (tc_common.cuh)
+    const char* gang_env = experiment_env("RMSYNTH_GANG");
     const int sync_lag = lag_env ? atoi(lag_env) : 0;
     int gang = gang_env ? atoi(gang_env) : T;
     if (gang < 1 || gang > T || T % gang) gang = T;
@@ -174,8 +174,8 @@ rmsynth_status tc_execute(const rmsynth_plan* p, const float* Q, const float* U,
     // (max |F|^2, k) per segment and peaks_gather_kernel reads the three samples around k* back from the cubes.
     int ring_out = 0;
     CUtensorMap mfq, mfu;
-    if (f16 && out_phi && FQ && !FA && !getenv("RMSYNTH_NO_RING_OUT")) {
-        const char* force = getenv("RMSYNTH_RING_OUT");      // EXPERIMENT knob: 1 = ring + TMA stores, 2 = vector stores
+    if (f16 && out_phi && FQ && !FA && !experiment_env("RMSYNTH_NO_RING_OUT")) {
+        const char* force = experiment_env("RMSYNTH_RING_OUT");   // experiment build only: 1 = ring + TMA stores, 2 = vector stores
         const int want = force ? atoi(force) : 1;
         if (want == 1 && n_pix % 4 == 0 && n_pix < (1LL << 31) && !((uintptr_t)FQ & 15) && !((uintptr_t)FU & 15)) ring_out = 1;
         else if (n_pix % 2 == 0 && !((uintptr_t)FQ & 7) && !((uintptr_t)FU & 7)) ring_out = 2;

@@ -128,6 +128,7 @@ struct Tc3Params {
     long long n_pix;
     int n_chan, n_phi, n, n_phi_tiles, n_chunks, n_items, n_pairs, a3d;
     float inv_scale_b;            // 2^-eB
+    int e_min;                    // 15 + eB: lowest chunk exponent whose drain factor 2^(e - 141 - eB) is a normal FP32
     const __half* blob;
     const uint32_t* chan_mask;    // [n_chunks] bit i: channel 32 c + i exists and has w > 0
     float* FQ;                    // may be NULL
@@ -442,9 +443,12 @@ tc3_rmsynth_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&raw_empty[sr]);         // every lane's loads have completed (values used above)
                 if (++sr == T3_R) { sr = 0; pr ^= 1; }
-                // scale 2^(141 - e) brings the chunk's largest sample into [2^14, 2^15); e clamped so both powers are normal
+                // scale 2^(141 - e) brings the chunk's largest sample into [2^14, 2^15); e clamped so that both powers AND the
+                // drain factor below are normal FP32 numbers.  A chunk whose maximum lies under the clamp (2^(eB - 112),
+                // ~1e-27) is scaled by the clamp's power instead: its halves sit lower in the FP16 range and lose
+                // precision gradually (2^-24 of the scaled value 1) instead of being flushed to zero by the factor.
                 int e = (int)(__float_as_uint(m) >> 23);
-                e = min(max(e, 15), 254);
+                e = min(max(e, prm.e_min), 254);
                 const float scale = __uint_as_float((uint32_t)(268 - e) << 23);
                 const uint64_t scale2 = pack2(scale, scale);
                 // what the epilogue multiplies the drained chunk with: 2^(e - 141) 2^-eB (B's plan-time scale folded in)
@@ -657,6 +661,7 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
     prm.n_items = prm.n_pairs * prm.n_phi_tiles;
     prm.a3d = a3d ? 1 : 0;
     prm.inv_scale_b = (float)std::ldexp(1.0, -p->tc3_eb);
+    prm.e_min = 15 + (p->tc3_eb > 0 ? p->tc3_eb : 0);
     prm.blob = reinterpret_cast<const __half*>(p->d_tcB3);
     prm.chan_mask = p->d_chanmask;
     prm.FQ = FQ;
@@ -670,7 +675,7 @@ rmsynth_status tc3_launch(const rmsynth_plan* p, const void* map_q, const void* 
         // one item lasts ~ n_chunks x 1350 cycles (12 MMAs of 104 cycles + overheads); spread the gangs over one item
         const int max_cl = p->sm_count / 2;
         const int S = (max_cl / gang) * gang, n_groups = S / gang + (max_cl - S);
-        const char* e = getenv("RMSYNTH_STAGGER");             // EXPERIMENT knob: percent of the default, 0 = off
+        const char* e = experiment_env("RMSYNTH_STAGGER");     // experiment build only: percent of the default, 0 = off
         const double scale = e ? atof(e) / 100.0 : 1.0;
         prm.stagger = (FQ || FA) && n_groups > 1 ? (int)(scale * prm.n_chunks * 1350.0 / n_groups) : 0;
     }
