@@ -19,7 +19,8 @@ def oracle_reference(oracle, nu, w, phi, q_los, u_los, lambda0_mode=0, lambda0_s
 
 def check_cubes(FQ_gpu, FU_gpu, FQ, FU, T, what=""):
     """FQ_gpu/FU_gpu: float32 [n_pix, n_phi] (already brought to LOS-major)."""
-    err = np.maximum(np.abs(FQ_gpu.astype(np.float64) - FQ), np.abs(FU_gpu.astype(np.float64) - FU)).max(axis=1)
+    # |F_gpu - F_oracle| of the complex samples (the north_star's quantity), not the larger of its two components
+    err = np.hypot(FQ_gpu.astype(np.float64) - FQ, FU_gpu.astype(np.float64) - FU).max(axis=1)
     Tsafe = np.where(T > 0, T, 1.0)
     ratio = err / Tsafe
     worst = float(ratio.max()) if ratio.size else 0.0

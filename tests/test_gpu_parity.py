@@ -212,6 +212,32 @@ def test_coherent_worst_case_and_dynamic_range(b, oracle_mod, scheme):
 
 
 @pytest.mark.parametrize("scheme", SCHEMES)
+def test_very_faint_cubes(b, oracle_mod, scheme):
+    """Samples far below any physical flux scale (FP32's smallest normal number is 1.2e-38): lines of sight whose largest
+    sample is 1e-24, 1e-26 and 1e-28 keep the parity tolerance in every scheme.  The FP16 scheme scales every 32-channel
+    chunk by its own maximum, floored at 2^(eB - 112) ~ 3e-27 so that the factor the epilogue multiplies back stays a
+    normal FP32 number; a chunk under the floor is scaled by the floor's power, its hi half (a multiple of 16 after
+    scaling) empties and the lo half carries it alone: accuracy falls off by a factor two per factor two, down to plain
+    FP16 (2^-12 per sample) -- never flushed to zero (rmsynth.h).  Lines of sight at 1e-31 check exactly that."""
+    cfg = ri.CONFIGS[5]
+    nu, w, phi = ri.grids(cfg)
+    q, u = ri.generate_pixels(cfg, torch.arange(7, 7 + 200))
+    scale = np.repeat([1e-24, 1e-26, 1e-28, 1e-31], 50)[:, None]
+    amp = np.maximum(np.abs(q.numpy()), np.abs(u.numpy())).max(axis=1, keepdims=True).astype(np.float64)   # per line of sight
+    q = (q.numpy().astype(np.float64) / amp * scale).astype(np.float32)
+    u = (u.numpy().astype(np.float64) / amp * scale).astype(np.float32)
+    _, FQ, FU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
+    assert T.min() > 1e-34
+    plan = b.Plan(nu, w, phi, scheme=scheme_ids(b)[scheme])
+    out = run_gpu(b, plan, q, u, "freq", "phi")
+    worst = check_cubes(out["FQ"][:150], out["FU"][:150], FQ[:150], FU[:150], T[:150], f"{scheme} faint")
+    err = np.hypot(out["FQ"][150:] - FQ[150:], out["FU"][150:] - FU[150:]).max(axis=1) / T[150:]
+    assert np.all(np.isfinite(err)) and err.max() <= (1e-3 if scheme == "f16x3" else TOL), f"{scheme} at 1e-31: {err.max():.2e} of T_p"
+    print(f"{scheme} faint cubes: max err/T_p = {worst:.2e} (1e-24 .. 1e-28), {err.max():.2e} (1e-31)")
+    plan.destroy()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
 def test_flagged_channels_full_of_interference(b, oracle_mod, scheme):
     """Reading A13: a zero-weight channel contributes nothing, whatever (finite) garbage it holds.  Samples of
     1e30 in flagged channels next to O(1) data must neither change the result nor cost accuracy (the FP16 split
@@ -588,7 +614,8 @@ def test_nonfinite_lines_of_sight_in_the_peak_maps(b, oracle_mod, scheme, lin, l
 def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id, scheme):
     """The cube bench.py times (same layouts, same scheme, one rmsynth_execute_peaks call over the whole
     cube), checked on lines of sight the oracle can compute one by one: every pixel of the first and last
-    tile, tile-boundary neighbours and a random sample; plus properties that hold at any size."""
+    tile pair, tile-boundary neighbours and 16 384 random lines of sight; plus properties that hold at any
+    size."""
     cfg = ri.CONFIGS[cfg_id]
     nu, w, phi = ri.grids(cfg)
     Q, U = ri.generate_cube(cfg, "cuda")
@@ -614,8 +641,11 @@ def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id, scheme):
     # sampled lines of sight against the oracle
     rng = np.random.default_rng(cfg_id)
     n = cfg.n_pix
-    pix = np.unique(np.concatenate([np.arange(0, 128), np.arange(n - 128, n), np.arange(127, n, max(n // 64, 128))[:64],
-                                    np.arange(128, n, max(n // 64, 128))[:64], rng.choice(n, 256, replace=False)]))
+    # 16 384 random lines of sight plus every pixel of the first and last tile pair (256 pixels: the FP16
+    # kernel's CTA pair owns 256) and both sides of 256 tile boundaries spread over the cube
+    edges = np.arange(128, n, 128)[:: max((n // 128) // 256, 1)][:256]
+    pix = np.unique(np.concatenate([np.arange(0, min(256, n)), np.arange(max(n - 256, 0), n), edges - 1, edges,
+                                    rng.choice(n, min(16384, n), replace=False)]))
     q, u = ri.gather_los(Q, U, cfg.layout_in, pix)
     op, oFQ, oFU, T = oracle_reference(oracle_mod, nu, w, phi, q, u)
     idx = torch.as_tensor(pix, device="cuda")
@@ -626,3 +656,42 @@ def test_full_size_cube_sampled_against_oracle(b, oracle_mod, cfg_id, scheme):
     check_peaks(oracle_mod, op, oFQ, oFU, T, got, cfg.dphi, f"full config {cfg_id}")
     print(f"full config {cfg_id}: {pix.size} sampled lines of sight, max err/T_p = {worst:.2e}")
     plan.destroy()
+
+
+@pytest.mark.parametrize("cfg_id", [5, 3])
+def test_full_size_cube_two_schemes_agree_everywhere(b, cfg_id):
+    """A supplement to the sampled oracle comparison above, not a substitute: the FP16X3 and 3xTF32 kernels share no
+    operand format, tile shape or work schedule, so a fault confined to one tile of either would show as a
+    disagreement somewhere in the cube.  Every sample of the full cube (configs[4], FITS order in / phi-major out, and
+    configs[2], LOS-major in and out, the largest by MACs) is compared on the device: |F_a - F_b| <= 2e-5 T_p, twice the
+    oracle tolerance each of them meets on the sampled lines of sight."""
+    cfg = ri.CONFIGS[cfg_id]
+    nu, w, phi = ri.grids(cfg)
+    Q, U = ri.generate_cube(cfg, "cuda")
+    layout = (b.IN_FREQ_MAJOR if cfg.layout_in == "freq" else 0) | (b.OUT_PHI_MAJOR if cfg.layout_out == "phi" else 0)
+    shape = (cfg.n_phi, cfg.n_pix) if cfg.layout_out == "phi" else (cfg.n_pix, cfg.n_phi)
+    out = {}
+    for name, scheme in (("f16x3", b.SCHEME_F16X3), ("tf32x3", b.SCHEME_TF32X3)):
+        FQ = torch.full(shape, float("nan"), device="cuda")
+        FU = torch.full(shape, float("nan"), device="cuda")
+        plan = b.Plan(nu, w, phi, scheme=scheme)
+        plan.execute(Q, U, cfg.n_pix, layout, FQ, FU)
+        torch.cuda.synchronize()
+        K = plan.K
+        plan.destroy()
+        out[name] = (FQ, FU)
+    kw = torch.as_tensor(K * w, dtype=torch.float32, device="cuda")
+    amp_in = torch.sqrt(Q * Q + U * U)
+    T_all = (amp_in * (kw[:, None] if cfg.layout_in == "freq" else kw[None, :])).sum(0 if cfg.layout_in == "freq" else 1)
+    del amp_in, Q, U
+    T_all = torch.where(T_all > 0, T_all, torch.ones_like(T_all))
+    worst = 0.0
+    (aq, au), (bq, bu) = out["f16x3"], out["tf32x3"]
+    step = 64 if cfg.layout_out == "phi" else 1 << 18      # depth planes / lines of sight per slice: bounded temporaries
+    for s0 in range(0, shape[0], step):
+        d = torch.hypot(aq[s0:s0 + step] - bq[s0:s0 + step], au[s0:s0 + step] - bu[s0:s0 + step])
+        d = d / (T_all[None, :] if cfg.layout_out == "phi" else T_all[s0:s0 + step, None])
+        assert bool(torch.isfinite(d).all()), f"config {cfg_id}: non-finite sample in slice {s0}"
+        worst = max(worst, float(d.max()))
+    print(f"full config {cfg_id}: FP16X3 vs 3xTF32 over all {shape[0] * shape[1]} samples, max |dF|/T_p = {worst:.2e}")
+    assert worst <= 2 * TOL
