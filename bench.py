@@ -31,7 +31,7 @@ sys.path.insert(0, ROOT)
 METRIC = "complex_GMAC_per_s"            # LOS x chan x phi complex multiply-accumulates per second / 1e9
 TENSOR_FLOP_PER_CMAC = 24.0              # 4 real products x 3 split passes x 2
 FP32_FLOP_PER_CMAC = 8.0
-NCU_FILE = os.path.join(ROOT, "profiles", "r02_ncu_summary.json")
+NCU_FILE = os.path.join(ROOT, "profiles", "r03_ncu_summary.json")
 
 
 def load_peaks():
@@ -489,13 +489,15 @@ def main():
                 "isolated": None if not isolated else dict(isolated, achieved=TENSOR_FLOP_PER_CMAC * cfg.cmac / (isolated["ms_median"] * 1e-3) / 1e12,
                                                            frac_of_burst_peak=TENSOR_FLOP_PER_CMAC * cfg.cmac / (isolated["ms_median"] * 1e-3) / 1e12 / peak),
                 "traffic": ev["dram_bytes"] if ev else None,
-                "tensor_pipe_active_pct_ncu": ev["tensor_pipe_active_pct"] if ev else None,
+                "tensor_pipe_pct_of_elapsed_cycles_ncu": ev["tensor_pipe_elapsed_pct"] if ev else None,
+                "tensor_pipe_pct_of_sm_active_cycles_ncu": ev["tensor_pipe_active_pct"] if ev else None,
+                "peaks_gather_ncu": ev.get("peaks_gather") if ev else None,
                 "kernel": "tc3_rmsynth_kernel" if f16 else "tc2_rmsynth_kernel",
                 "note": f"executed split-precision tensor FLOP (3 products x 4 real x 2 = 24 per useful complex MAC) / mean CUDA-event "
                         f"step time; peak = {peaks_src} bf16 BURST {peaks['bf16_tflops']:.0f} TF ({'fp16 = bf16 rate' if f16 else 'tf32'}); the "
                         f"timed region is {a.steps} back-to-back {kern_ms:.1f} ms kernels under the 1 kW power cap (see clocks), where the same "
                         f"file's SUSTAINED figure {peaks.get('bf16_tflops_sustained', 0):.0f} TF applies: frac_of_sustained_peak; traffic and "
-                        f"tensor_pipe_active_pct_ncu come from profiles/r02_ncu_summary.json and are null unless that capture was taken "
+                        f"the tensor_pipe_* / peaks_gather_ncu fields come from profiles/r03_ncu_summary.json and are null unless that capture was taken "
                         f"with these very tensor-path sources (content hash {tensor_path_hash()}; library {src_hash})"}
     else:
         achieved = FP32_FLOP_PER_CMAC * cfg.cmac / (kern_ms * 1e-3) / 1e12

@@ -72,17 +72,17 @@ def test_product_path_never_imports_the_oracle():
 
 
 def test_committed_ncu_evidence_belongs_to_the_committed_tensor_sources():
-    """bench.py quotes `traffic` and the tensor-pipe activity from profiles/r02_ncu_summary.json only when that capture was
+    """bench.py quotes `traffic` and the tensor-pipe activity from profiles/r03_ncu_summary.json only when that capture was
     taken with the tensor-path sources that run; a kernel edit without a new capture must not go unnoticed."""
     import importlib.util
     import json
     spec = importlib.util.spec_from_file_location("bench_module", os.path.join(ROOT, "bench.py"))
     bench = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(bench)
-    with open(os.path.join(ROOT, "profiles", "r02_ncu_summary.json")) as f:
+    with open(os.path.join(ROOT, "profiles", "r03_ncu_summary.json")) as f:
         captures = json.load(f)["captures"]
     assert "5:f16x3" in captures
     for key, e in captures.items():
-        assert e["tensor_path_hash"] == bench.tensor_path_hash(), f"{key}: re-capture with ncu (profiles/r02_ncu_tc3.md names the commands)"
-        assert e["dram_bytes"] > 0 and 0 < e["tensor_pipe_active_pct"] <= 100
+        assert e["tensor_path_hash"] == bench.tensor_path_hash(), f"{key}: re-capture with ncu (profiles/r03_ncu_kernels.md names the commands)"
+        assert e["dram_bytes"] > 0 and 0 < e["tensor_pipe_elapsed_pct"] <= e["tensor_pipe_active_pct"] <= 100
     assert bench.ncu_evidence(5, "f16x3") is not None
